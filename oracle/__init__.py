@@ -1,0 +1,6 @@
+"""fp64 CPU oracle of the APIC closed-form reconstruction.  TEST INFRASTRUCTURE ONLY.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  It shares no code with
+``paper_2407_20469_b200`` (the CUDA product path) and imports nothing from it.
+"""

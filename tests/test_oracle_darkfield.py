@@ -1,0 +1,153 @@
+"""Pins for the darkfield extension O6 (Eq. 11-13) and the outputs O7."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+from apic_synth import get_config, make_tile
+from oracle import apic_oracle as O
+from helpers import oracle_params, read_golden_table, rel_l2, truth_object_spectrum
+
+
+def _small_cfg(n=64):
+    return get_config(2, tile_n=n, batch=4, grid=(2, 2))
+
+
+def test_correlation_by_fft_equals_double_sum():
+    rng = np.random.default_rng(7)
+    n = 32
+    a = np.zeros((n, n), complex)
+    b = np.zeros((n, n), complex)
+    a[10:20, 12:19] = rng.standard_normal((10, 7)) + 1j * rng.standard_normal((10, 7))
+    b[13:18, 9:21] = rng.standard_normal((5, 12)) + 1j * rng.standard_normal((5, 12))
+    at = np.zeros((n, n), bool)
+    at[8:26, 6:27] = True
+    direct = O.correlate_direct(a, b, at)
+    fast = O.correlate_fft(a, b)
+    assert np.abs(direct[at] - fast[at]).max() < 1e-12
+
+
+def test_minkowski_difference_small():
+    a = np.zeros((16, 16), bool)
+    b = np.zeros((16, 16), bool)
+    a[9, 10] = a[9, 11] = True         # bins (2,1), (3,1)
+    b[8, 8] = b[7, 8] = True           # bins (0,0), (0,-1)
+    d = O.minkowski_difference(a, b)
+    got = {(int(x) - 8, int(y) - 8) for y, x in zip(*np.nonzero(d))}
+    assert got == {(2, 1), (3, 1), (2, 2), (3, 2)}
+
+
+def test_index_set_sizes_match_survey_n256():
+    g = [r for r in read_golden_table("geometry_counts.txt") if r[0] == "cfg1_2_4"][0]
+    cfg = get_config(2)
+    geo = O.Geometry(oracle_params(cfg))
+    sets, known = O.darkfield_sets(geo)
+    assert [s.led for s in sets] == list(range(16))          # ascending |kappa|, ties by input order
+    assert int(known.sum()) == int(g[8])
+    assert (int(sets[0].U.sum()), int(sets[0].Q.sum())) == (int(g[9]), int(g[10]))
+    assert (int(sets[8].U.sum()), int(sets[8].Q.sum())) == (int(g[11]), int(g[12]))
+    assert max(s.unknown_fraction for s in sets) < 0.23      # 8-10 % / 21-22 %
+    for s in sets:                                           # Q excludes the origin-side regions
+        assert not s.Q[cfg.tile_n // 2, cfg.tile_n // 2]
+        mirrored = np.zeros_like(s.Q)                        # Q and -Q are disjoint
+        mirrored[1:, 1:] = s.Q[1:, 1:][::-1, ::-1]
+        assert not (s.Q & mirrored).any()
+
+
+def test_too_large_unknown_fraction_is_rejected():
+    cfg = get_config(2, tile_n=64, dark_rings=((0.48, 8),))
+    geo = O.Geometry(oracle_params(cfg))
+    with pytest.raises(ValueError, match="unknown fraction"):
+        O.darkfield_sets(geo)
+
+
+def test_dark_order_ascending_kappa_ties_by_input_order():
+    cfg = get_config(2, tile_n=64, dark_rings=((0.40, 8), (0.30, 8)))   # outer ring listed first
+    geo = O.Geometry(oracle_params(cfg))
+    assert geo.dark_order == list(range(8, 16)) + list(range(0, 8))
+
+
+def test_exact_unknown_spectrum_from_exact_known_spectrum():
+    """Exact result (Eq. 13): given the true known spectrum and pupil, every darkfield LED's
+    least-squares solution equals the true unknown spectrum."""
+    cfg = _small_cfg(64)
+    _, truth = make_tile(cfg, 1, noise="none", keep_clean=True)
+    p = oracle_params(cfg)
+    geo = O.Geometry(p)
+    target = truth_object_spectrum(cfg, truth, geo.radius)
+    bf = np.zeros((64, 64), bool)
+    for m in geo.disc_b:
+        bf |= m
+    ct = np.array([truth.coef[j] for j in cfg.noll_fit])
+    info = []
+    o_hat, known = O.darkfield_extend(geo, np.where(bf, target, 0), bf, ct,
+                                      truth.clean[cfg.n_bright:], collect=info)
+    assert int(known.sum()) > int(bf.sum())
+    assert rel_l2(o_hat[known & ~bf], target[known & ~bf]) < 1e-10
+    assert max(i["resid"] for i in info) < 1e-10             # consistent system: zero residual
+    # the matrix is well conditioned (SURVEY: cond(C) 1.8-9.2) and has full column rank
+    ds = O.darkfield_sets(geo)[0][0]
+    phi = O.pupil_phase(p.noll, ct, geo.kx, geo.ky, geo.kappa_d[ds.led], geo.radius)
+    cmat = O.darkfield_matrix(np.where(ds.P, target * np.exp(1j * phi), 0), ds.P, ds.U, ds.Q)
+    sv = np.linalg.svd(cmat, compute_uv=False)
+    assert sv[-1] > 0 and sv[0] / sv[-1] < 12
+
+
+def test_darkfield_matrix_is_the_correlation_operator():
+    cfg = _small_cfg(64)
+    geo = O.Geometry(oracle_params(cfg))
+    ds = O.darkfield_sets(geo)[0][3]
+    rng = np.random.default_rng(11)
+    p_hat = np.where(ds.P, rng.standard_normal((64, 64)) + 1j * rng.standard_normal((64, 64)), 0)
+    u = np.zeros((64, 64), complex)
+    u[ds.U] = rng.standard_normal(int(ds.U.sum())) + 1j * rng.standard_normal(int(ds.U.sum()))
+    cmat = O.darkfield_matrix(p_hat, ds.P, ds.U, ds.Q)
+    direct = O.correlate_direct(u, p_hat, ds.Q)              # [U ⋆ P](k) = sum_q U(q+k) conj P(q)
+    assert np.abs(cmat @ u[ds.U] - direct[ds.Q]).max() < 1e-12
+    # and on Q the other two terms of Eq. 12 vanish identically (that is what defines Q, R16)
+    assert np.abs(O.correlate_direct(p_hat, u, ds.Q)[ds.Q]).max() == 0
+    assert np.abs(O.correlate_direct(u, u, ds.Q)[ds.Q]).max() == 0
+
+
+def test_full_pipeline_noise_free_64_matches_ground_truth():
+    """SURVEY pin: 64^2, 8 + 16 LEDs, noise-free, kk_pad 2: ~4e-8 over the whole synthetic band."""
+    cfg = _small_cfg(64)
+    _, truth = make_tile(cfg, 0, noise="none", keep_clean=True)
+    p = oracle_params(cfg, kk_pad=2)
+    r = O.reconstruct_tile(truth.clean, p, keep=True)
+    target = truth_object_spectrum(cfg, truth, p.radius)
+    assert r.status == O.STATUS_OK
+    assert int(r.known.sum()) == 2221
+    assert rel_l2(r.o_hat[r.known], target[r.known]) < 1e-6
+    assert np.all(r.o_hat[~r.known] == 0)
+    # synthetic aperture reach (NA_ill,max + NA)/lambda: outermost known bin (27.5 of 32)
+    reach = np.hypot(*np.nonzero(r.known)[::-1] - np.array([[32], [32]])).max()
+    assert 27.0 < reach < 28.0
+    # the output field is the band-limited truth on the 3x grid, blank -> 1 normalisation
+    assert rel_l2(r.field, O.output_field(np.where(r.known, target, 0), 3)) < 1e-6
+
+
+def test_output_field_conventions():
+    n, u = 16, 3
+    o = np.zeros((n, n), complex)
+    o[n // 2, n // 2] = 1.0                       # blank object
+    assert np.abs(O.output_field(o, u) - 1.0).max() < 1e-14
+    o[n // 2 + 2, n // 2 - 3] = 0.5j              # bin (kx, ky) = (-3, 2)
+    X = np.arange(n * u)
+    want = 1.0 + 0.5j * np.exp(2j * np.pi * (-3 * X[None, :] + 2 * X[:, None]) / (n * u))
+    assert np.abs(O.output_field(o, u) - want).max() < 1e-13
+
+
+def test_background_and_bad_input_status():
+    cfg = get_config(4, batch=16, grid=(4, 4))
+    p = oracle_params(dataclasses.replace(cfg, tile_n=64), bg_mode=1, bg_threshold=0.9)
+    small = dataclasses.replace(cfg, tile_n=64)
+    blank, _ = make_tile(small, 0, blank=True)
+    r = O.reconstruct_tile(blank, p)
+    assert r.status == O.STATUS_BACKGROUND and not r.field.any() and not r.zernike.any()
+    sample, _ = make_tile(small, 1, blank=False)
+    assert not O.background_flag(sample[:8], 1, 0.9)
+    assert O.background_flag(blank[:8], 2, 1e-2) and not O.background_flag(sample[:8], 2, 1e-2)
+    bad = sample.copy()
+    bad[3, 5, 7] = np.nan
+    assert O.reconstruct_tile(bad, p).status == O.STATUS_BAD_INPUT
