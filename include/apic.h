@@ -1,0 +1,167 @@
+/* apic.h - C ABI of libapic: B200-native APIC closed-form reconstruction.
+ *
+ * The operation is the per-tile reconstruction of arXiv 2407.20469 (§2.3, lines 64-135,
+ * Fig. 2 at line 70): a stack of intensity images I_i taken under NA-matching and darkfield LED
+ * illumination is turned into an aberration-corrected complex field on an upsampled grid plus the
+ * tile's recovered pupil.  Steps, each executed by hand-written sm_100a kernels:
+ *   S0     background flag (BASELINE.json item 5)
+ *   S1-S5  Kramers-Kronig field retrieval, Eq. 4-7
+ *   S6     aberration extraction from phase differences in overlaps, Eq. 8-10,
+ *          in a Noll-Zernike basis, weighted normal equations + Cholesky (BASELINE.json item 3)
+ *   S7     correction + stitching
+ *   S8-S10 darkfield extension, Eq. 11-13, matrix-free CGLS on C u = d
+ *   S10    zero-padded inverse transform to the u*N grid, pupil output
+ * Readings of the silent / garbled points are DESIGN.md §3 (R1-R23 of SURVEY.md §8(c)).
+ *
+ * Conventions: images and fields are row-major [y][x], x fastest; the spatial origin is pixel
+ * (0,0); raw pixel m maps to output pixel u*m; spectra are normalised so that DC = spatial mean.
+ * A blank object (amplitude 1, phase 0) gives I = 1 in every NA-matching image and a field = 1.
+ *
+ * All functions return 0 (APIC_OK) on success and a negative apic_error otherwise.  No exceptions
+ * cross the boundary, there is no global state and no CPU fallback: if no CUDA device is usable the
+ * calls fail with APIC_ECUDA.  A plan is not thread-safe; use one plan per stream.
+ */
+#ifndef APIC_H_
+#define APIC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct apic_plan apic_plan; /* opaque; owns all device tables and the workspace */
+
+typedef enum {
+  APIC_OK = 0,
+  APIC_EINVAL = -1,   /* bad parameter / geometry (see apic_plan_create) */
+  APIC_ECUDA = -2,    /* a CUDA runtime call failed (apic_last_cuda_error gives the text) */
+  APIC_ENOMEM = -3,   /* host or device allocation failed */
+  APIC_EBATCH = -4    /* batch outside 1..max_batch */
+} apic_error;
+
+/* Per-tile status written to d_status. */
+enum {
+  APIC_TILE_OK = 0,
+  APIC_TILE_BACKGROUND = 1, /* skipped by the background criterion; outputs are zero          */
+  APIC_TILE_BAD_INPUT = 2,  /* a non-finite input pixel; outputs are zero                     */
+  APIC_TILE_SOLVE_FAILED = 3 /* weighted phase residual of the aberration fit > 1 rad RMS (or
+                                non-finite); outputs are still written                        */
+};
+
+typedef struct {
+  int tile_n;            /* N: raw tile side, 64 | 128 | 256 | 512                               */
+  int upsample;          /* u: 1..4, output grid is (u*N)^2                                       */
+  double wavelength_um;  /* lambda                                                              */
+  double pixel_um;       /* effective pixel = camera pitch / magnification         */
+  double na_obj;         /* objective NA                                                        */
+  int n_bright;          /* number of NA-matching LEDs (>= 3)                                    */
+  const double* k_bright;/* host, [n_bright][2] (kx,ky) in cycles/um, |k| = NA/lambda*/
+  int n_dark;            /* number of darkfield LEDs (may be 0)                                  */
+  const double* k_dark;  /* host, [n_dark][2], |k| > NA/lambda; NULL if n_dark == 0               */
+  int n_zernike;         /* number of fitted Zernike terms (1..64)                               */
+  const int* noll;       /* host, [n_zernike] distinct Noll indices, each >= 4 (piston and tilts
+                            are the exact null space of Eq. 10; R9)                    */
+  int kk_pad;            /* Fourier pre-upsampling of I before the log: only 1 is implemented     */
+  int refine_iters;      /* re-wrapped refinements of the aberration fit (R11); 0..16   */
+  int df_iters;          /* maximum CGLS iterations per darkfield LED (>= 1)                      */
+  float df_tol;          /* CGLS stops when ||C^H r|| <= df_tol * ||C^H d||; 0 = run df_iters     */
+  float intensity_floor; /* I <- max(I, floor * mean(I)) before the log (R6)            */
+  int bg_mode;           /* 0 off | 1: mean(I_bright) >= bg_threshold | 2: var/mean^2 <= thr      */
+  float bg_threshold;
+  int max_batch;         /* apic_reconstruct accepts 1..max_batch tiles; workspace is sized for
+                            min(max_batch, internal chunk)                                       */
+  int chunk_tiles;       /* tiles per internal pass; 0 = chosen so that one pass's transform
+                            working set stays inside the 126 MB L2                              */
+} apic_params;
+
+/* Fills *p with the defaults (kk_pad 1, refine_iters 3, df_iters 48, df_tol 1e-6, floor 1e-6,
+ * bg off, max_batch 64); the caller then sets the geometry fields. */
+void apic_params_default(apic_params* p);
+
+/* Builds every geometry-only table on the host in fp64 (disc masks, half-plane weights of Eq. 5,
+ * overlap sets S_il of Eq. 8 and the rows of Eq. 10, darkfield sets P/U/Q of Eq. 13, Zernike
+ * tables, FFT twiddles), uploads them to the current CUDA device and allocates the workspace.
+ * The arrays inside *p are copied.  APIC_EINVAL if: N not in {64,128,256,512}; u outside 1..4;
+ * an NA-matching LED with | |kappa_i| - R | > 0.5 bin; the synthetic aperture does not fit the raw
+ * grid (max|kappa| + R >= N/2 - 1); a darkfield LED whose unknown fraction exceeds 42 %
+ * or whose linear region Q is empty; a Noll index < 4 or repeated; kk_pad != 1; fewer than one
+ * overlapping pair. */
+int apic_plan_create(const apic_params* p, apic_plan** out);
+int apic_plan_destroy(apic_plan* plan);
+
+typedef struct {
+  int tile_n, upsample, out_n;    /* out_n = u*N                                                */
+  int n_bright, n_dark, n_zernike;
+  int n_pairs;                    /* overlapping NA-matching pairs (Eq. 8)                       */
+  int n_rows, n_grad_rows;        /* rows of Eq. 10 / of the gradient-domain initialisation      */
+  int n_union;                    /* bins covered by the NA-matching discs                       */
+  int n_known;                    /* bins of the final extended spectrum                         */
+  int n_dark_used;                /* darkfield LEDs with a non-empty unknown set                 */
+  int max_unknown, max_equations; /* max |U_i|, max |Q_i|                                        */
+  int chunk_tiles;                /* tiles processed per internal pass                          */
+  size_t table_bytes, workspace_bytes;
+  double radius_bins;             /* R = NA*N*dx/lambda                                          */
+} apic_plan_info_t;
+int apic_plan_info(const apic_plan* plan, apic_plan_info_t* info);
+
+/* The same geometry numbers computed on the host only (no CUDA device is touched; table_bytes,
+ * workspace_bytes and chunk_tiles are 0).  If led / n_unknown / n_equations are non-NULL they
+ * receive up to `cap` darkfield index-set sizes in processing order.  Used by the CPU tests. */
+int apic_geometry_info(const apic_params* p, apic_plan_info_t* info, int* led, int* n_unknown,
+                       int* n_equations, int cap);
+
+/* Darkfield index-set sizes in processing order (ascending |kappa|, ties by input order):
+ * led[k] = input index, n_unknown[k] = |U|, n_equations[k] = |Q|.  Arrays hold n_dark_used ints. */
+int apic_plan_dark_sets(const apic_plan* plan, int* led, int* n_unknown, int* n_equations);
+
+/* The whole hot path for `batch` tiles.  Every pointer is a DEVICE pointer owned by the caller;
+ * all work is enqueued on `cuda_stream` (a cudaStream_t, NULL = legacy default stream).  With
+ * bg_mode == 0 the call returns without synchronising; with bg_mode != 0 it synchronises the
+ * stream once, after the background pass, to read the number of tiles left to reconstruct.
+ *   d_intensity [batch][n_bright+n_dark][N][N] float, NA-matching images first, LED order = plan
+ *               order, common radiometric units (R17)
+ *   d_field     [batch][uN][uN] complex64 as (re,im) float pairs
+ *   d_zernike   [batch][n_zernike] float, rad, Noll-normalised, order = plan's noll[]
+ *   d_pupil     [batch][N][N] complex64, 1[|k|<=R] exp(j phi_hat(k)), centred (bin 0 at N/2); or NULL
+ *   d_status    [batch] int32, APIC_TILE_*
+ */
+int apic_reconstruct(apic_plan* plan, const float* d_intensity, int batch, float* d_field,
+                     float* d_zernike, float* d_pupil, int32_t* d_status, void* cuda_stream);
+
+/* Same call with HOST buffers (pinned or pageable): copies the inputs to the device, runs
+ * apic_reconstruct, copies the results back and synchronises the stream before returning.
+ * h_pupil may be NULL. */
+int apic_reconstruct_host(apic_plan* plan, const float* h_intensity, int batch, float* h_field,
+                          float* h_zernike, float* h_pupil, int32_t* h_status, void* cuda_stream);
+
+/* Stage-level access for parity tests (device pointers, valid after apic_reconstruct on the
+ * same stream, for the tiles of the LAST internal chunk; tile index is chunk-local):
+ *   APIC_DBG_SUBSPECTRA: [chunk][sum_i |D_i|] complex64, S_hat_i on D_i (Eq. 7), LED-major, bins
+ *                        of each disc in row-major order of the centred grid
+ *   APIC_DBG_OBJECT_SPECTRUM: [chunk][N][N] complex64, O_hat in FFT order (bin k at index k mod N)
+ *   APIC_DBG_DF_ITERS:   [chunk][n_dark_used] int32, CGLS iterations actually run
+ */
+enum { APIC_DBG_SUBSPECTRA = 0, APIC_DBG_OBJECT_SPECTRUM = 1, APIC_DBG_DF_ITERS = 2 };
+int apic_debug_buffer(const apic_plan* plan, int which, void** d_ptr, size_t* bytes_per_tile);
+/* Copies `tiles` tiles of that buffer into the caller's device buffer d_dst (asynchronously, on
+ * cuda_stream). */
+int apic_debug_copy(const apic_plan* plan, int which, void* d_dst, int tiles, void* cuda_stream);
+
+/* Batched 2-D complex FFT used by every stage, exposed for kernel-level parity tests:
+ * d_data [batch][n][n] complex64 transformed in place; forward = unnormalised e^{-j..}, inverse =
+ * unnormalised e^{+j..}.  n in {64,128,256,512}. */
+int apic_fft2d(float* d_data, int n, int batch, int inverse, void* cuda_stream);
+
+/* Number of kernels launched by the last apic_reconstruct on this plan (bench's gpu_launches). */
+int apic_last_launch_count(const apic_plan* plan);
+
+const char* apic_strerror(int err);
+const char* apic_last_cuda_error(void);
+const char* apic_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* APIC_H_ */

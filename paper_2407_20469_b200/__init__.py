@@ -1,0 +1,234 @@
+"""Thin Python binding of libapic (include/apic.h): argument marshalling only.
+
+Every step of the reconstruction runs in the CUDA kernels of ``libapic.so``; PyTorch supplies
+device memory and streams.  There is no CPU fallback: importing works without a GPU (so the
+symbol table and the host-only geometry can be tested), but ``Plan(...)`` raises ``ApicError``
+when no CUDA device is usable, and a missing ``libapic.so`` raises at ``load()``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+from typing import Optional, Sequence
+
+import numpy as np
+
+_PKG = Path(__file__).resolve().parent
+LIB_PATH = _PKG / "libapic.so"
+
+APIC_OK, APIC_EINVAL, APIC_ECUDA, APIC_ENOMEM, APIC_EBATCH = 0, -1, -2, -3, -4
+TILE_OK, TILE_BACKGROUND, TILE_BAD_INPUT, TILE_SOLVE_FAILED = 0, 1, 2, 3
+DBG_SUBSPECTRA, DBG_OBJECT_SPECTRUM, DBG_DF_ITERS = 0, 1, 2
+
+EXPORTS = ("apic_params_default", "apic_plan_create", "apic_plan_destroy", "apic_plan_info",
+           "apic_geometry_info", "apic_plan_dark_sets", "apic_reconstruct", "apic_reconstruct_host",
+           "apic_debug_buffer", "apic_debug_copy", "apic_fft2d", "apic_last_launch_count", "apic_strerror",
+           "apic_last_cuda_error", "apic_version")
+
+
+class ApicError(RuntimeError):
+    pass
+
+
+class ApicParams(C.Structure):
+    _fields_ = [("tile_n", C.c_int), ("upsample", C.c_int), ("wavelength_um", C.c_double),
+                ("pixel_um", C.c_double), ("na_obj", C.c_double), ("n_bright", C.c_int),
+                ("k_bright", C.POINTER(C.c_double)), ("n_dark", C.c_int), ("k_dark", C.POINTER(C.c_double)),
+                ("n_zernike", C.c_int), ("noll", C.POINTER(C.c_int)), ("kk_pad", C.c_int),
+                ("refine_iters", C.c_int), ("df_iters", C.c_int), ("df_tol", C.c_float),
+                ("intensity_floor", C.c_float), ("bg_mode", C.c_int), ("bg_threshold", C.c_float),
+                ("max_batch", C.c_int), ("chunk_tiles", C.c_int)]
+
+
+class PlanInfo(C.Structure):
+    _fields_ = [("tile_n", C.c_int), ("upsample", C.c_int), ("out_n", C.c_int), ("n_bright", C.c_int),
+                ("n_dark", C.c_int), ("n_zernike", C.c_int), ("n_pairs", C.c_int), ("n_rows", C.c_int),
+                ("n_grad_rows", C.c_int), ("n_union", C.c_int), ("n_known", C.c_int), ("n_dark_used", C.c_int),
+                ("max_unknown", C.c_int), ("max_equations", C.c_int), ("chunk_tiles", C.c_int),
+                ("table_bytes", C.c_size_t), ("workspace_bytes", C.c_size_t), ("radius_bins", C.c_double)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+_lib = None
+
+
+def load() -> C.CDLL:
+    """dlopen libapic.so (built by ``python -m paper_2407_20469_b200.build``)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not LIB_PATH.exists():
+        raise ApicError(f"{LIB_PATH} is missing: build it with `python -m paper_2407_20469_b200.build` "
+                        "(CUDA-only library, no CPU fallback)")
+    lib = C.CDLL(str(LIB_PATH))
+    lib.apic_params_default.argtypes = [C.POINTER(ApicParams)]
+    lib.apic_params_default.restype = None
+    lib.apic_plan_create.argtypes = [C.POINTER(ApicParams), C.POINTER(C.c_void_p)]
+    lib.apic_plan_destroy.argtypes = [C.c_void_p]
+    lib.apic_plan_info.argtypes = [C.c_void_p, C.POINTER(PlanInfo)]
+    lib.apic_geometry_info.argtypes = [C.POINTER(ApicParams), C.POINTER(PlanInfo), C.POINTER(C.c_int),
+                                       C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_int]
+    lib.apic_plan_dark_sets.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int)]
+    lib.apic_reconstruct.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
+                                     C.c_void_p, C.c_void_p]
+    lib.apic_reconstruct_host.argtypes = lib.apic_reconstruct.argtypes
+    lib.apic_debug_buffer.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)]
+    lib.apic_debug_copy.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p]
+    lib.apic_fft2d.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
+    lib.apic_last_launch_count.argtypes = [C.c_void_p]
+    for name in ("apic_strerror", "apic_last_cuda_error", "apic_version"):
+        getattr(lib, name).restype = C.c_char_p
+    lib.apic_strerror.argtypes = [C.c_int]
+    _lib = lib
+    return lib
+
+
+def _check(rc: int, what: str):
+    if rc != APIC_OK:
+        lib = load()
+        msg = lib.apic_strerror(rc).decode()
+        if rc == APIC_ECUDA:
+            msg += ": " + lib.apic_last_cuda_error().decode()
+        raise ApicError(f"{what} failed ({rc}): {msg}")
+
+
+def make_params(tile_n: int, upsample: int, wavelength_um: float, pixel_um: float, na_obj: float,
+                k_bright, k_dark, noll: Sequence[int], **opts):
+    """Returns (ApicParams, keep-alive tuple).  ``opts``: kk_pad, refine_iters, df_iters, df_tol,
+    intensity_floor, bg_mode, bg_threshold, max_batch, chunk_tiles."""
+    lib = load()
+    p = ApicParams()
+    lib.apic_params_default(C.byref(p))
+    kb = np.ascontiguousarray(np.asarray(k_bright, dtype=np.float64).reshape(-1, 2))
+    kd = np.ascontiguousarray(np.asarray(k_dark if k_dark is not None else [], dtype=np.float64).reshape(-1, 2))
+    nl = np.ascontiguousarray(np.asarray(list(noll), dtype=np.int32))
+    p.tile_n, p.upsample = int(tile_n), int(upsample)
+    p.wavelength_um, p.pixel_um, p.na_obj = float(wavelength_um), float(pixel_um), float(na_obj)
+    p.n_bright, p.k_bright = kb.shape[0], kb.ctypes.data_as(C.POINTER(C.c_double))
+    p.n_dark = kd.shape[0]
+    p.k_dark = kd.ctypes.data_as(C.POINTER(C.c_double)) if kd.shape[0] else None
+    p.n_zernike, p.noll = nl.shape[0], nl.ctypes.data_as(C.POINTER(C.c_int))
+    for k, v in opts.items():
+        if not hasattr(p, k):
+            raise TypeError(f"unknown apic_params field {k!r}")
+        setattr(p, k, v)
+    return p, (kb, kd, nl)
+
+
+def geometry_info(params: ApicParams, max_dark: int = 256):
+    """Host-only geometry counts (no GPU needed): (info dict, [(led, |U|, |Q|), ...])."""
+    lib = load()
+    info = PlanInfo()
+    led = (C.c_int * max_dark)()
+    nu = (C.c_int * max_dark)()
+    nq = (C.c_int * max_dark)()
+    _check(lib.apic_geometry_info(C.byref(params), C.byref(info), led, nu, nq, max_dark), "apic_geometry_info")
+    n = min(info.n_dark_used, max_dark)
+    return info.as_dict(), [(led[i], nu[i], nq[i]) for i in range(n)]
+
+
+class Plan:
+    """apic_plan wrapper.  Tensors are torch CUDA tensors; the current torch stream is used."""
+
+    def __init__(self, tile_n, upsample, wavelength_um, pixel_um, na_obj, k_bright, k_dark, noll, **opts):
+        self._lib = load()
+        self.params, self._keep = make_params(tile_n, upsample, wavelength_um, pixel_um, na_obj, k_bright,
+                                              k_dark, noll, **opts)
+        self._h = C.c_void_p()
+        _check(self._lib.apic_plan_create(C.byref(self.params), C.byref(self._h)), "apic_plan_create")
+        info = PlanInfo()
+        _check(self._lib.apic_plan_info(self._h, C.byref(info)), "apic_plan_info")
+        self.info = info.as_dict()
+        self.n, self.u, self.out_n = info.tile_n, info.upsample, info.out_n
+        self.n_img = info.n_bright + info.n_dark
+        self.nz = info.n_zernike
+
+    @classmethod
+    def from_config(cls, cfg, **opts):
+        """cfg: apic_synth.ApicConfig-like object (tile_n, upsample, optics, noll_fit)."""
+        from apic_synth.configs import led_kvectors   # input recipe only, no method arithmetic
+        kb, kd = led_kvectors(cfg)
+        return cls(cfg.tile_n, cfg.upsample, cfg.wavelength_um, cfg.pixel_um, cfg.na_obj, kb, kd,
+                   cfg.noll_fit, **opts)
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.apic_plan_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def dark_sets(self):
+        n = self.info["n_dark_used"]
+        led, nu, nq = (C.c_int * max(n, 1))(), (C.c_int * max(n, 1))(), (C.c_int * max(n, 1))()
+        _check(self._lib.apic_plan_dark_sets(self._h, led, nu, nq), "apic_plan_dark_sets")
+        return [(led[i], nu[i], nq[i]) for i in range(n)]
+
+    def reconstruct(self, intensity, want_pupil: bool = True, out=None):
+        """intensity: float32 CUDA tensor [B][n_img][N][N].  Returns (field complex64 [B][uN][uN],
+        zernike float32 [B][nz], pupil complex64 [B][N][N] | None, status int32 [B])."""
+        import torch
+        if not (intensity.is_cuda and intensity.dtype == torch.float32 and intensity.is_contiguous()):
+            raise ApicError("intensity must be a contiguous float32 CUDA tensor")
+        b = intensity.shape[0]
+        if tuple(intensity.shape[1:]) != (self.n_img, self.n, self.n):
+            raise ApicError(f"intensity shape {tuple(intensity.shape)} != [B,{self.n_img},{self.n},{self.n}]")
+        dev = intensity.device
+        if out is None:
+            field = torch.empty((b, self.out_n, self.out_n), dtype=torch.complex64, device=dev)
+            zern = torch.empty((b, self.nz), dtype=torch.float32, device=dev)
+            pupil = torch.empty((b, self.n, self.n), dtype=torch.complex64, device=dev) if want_pupil else None
+            status = torch.empty((b,), dtype=torch.int32, device=dev)
+        else:
+            field, zern, pupil, status = out
+        stream = torch.cuda.current_stream(dev).cuda_stream
+        _check(self._lib.apic_reconstruct(self._h, intensity.data_ptr(), b, field.data_ptr(), zern.data_ptr(),
+                                          pupil.data_ptr() if pupil is not None else None, status.data_ptr(),
+                                          C.c_void_p(stream)), "apic_reconstruct")
+        return field, zern, pupil, status
+
+    def reconstruct_host(self, intensity, field, zern, pupil, status, stream: int = 0):
+        """Host buffers (numpy arrays or CPU torch tensors, ideally pinned); blocking."""
+        def ptr(a):
+            if a is None:
+                return None
+            return a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr()
+        b = intensity.shape[0]
+        _check(self._lib.apic_reconstruct_host(self._h, ptr(intensity), b, ptr(field), ptr(zern), ptr(pupil),
+                                               ptr(status), C.c_void_p(stream)), "apic_reconstruct_host")
+
+    def debug_buffer(self, which: int, tiles: int):
+        """Stage-level buffers of the last chunk as torch tensors (copies)."""
+        import torch
+        p, nbytes = C.c_void_p(), C.c_size_t()
+        _check(self._lib.apic_debug_buffer(self._h, which, C.byref(p), C.byref(nbytes)), "apic_debug_buffer")
+        total = nbytes.value * tiles
+        out = torch.empty(total, dtype=torch.uint8, device="cuda")
+        stream = torch.cuda.current_stream().cuda_stream
+        _check(self._lib.apic_debug_copy(self._h, which, out.data_ptr(), tiles, C.c_void_p(stream)),
+               "apic_debug_copy")
+        if which == DBG_DF_ITERS:
+            return out.view(torch.int32).view(tiles, -1)
+        return out.view(torch.complex64).view(tiles, -1)
+
+    @property
+    def last_launch_count(self) -> int:
+        return int(self._lib.apic_last_launch_count(self._h))
+
+
+def fft2d(x, inverse: bool = False):
+    """In-place batched 2-D FFT of a complex64 CUDA tensor [B][n][n] by the library's own kernels."""
+    import torch
+    if not (x.is_cuda and x.dtype == torch.complex64 and x.is_contiguous() and x.dim() == 3
+            and x.shape[1] == x.shape[2]):
+        raise ApicError("x must be a contiguous complex64 CUDA tensor [B][n][n]")
+    lib = load()
+    stream = torch.cuda.current_stream(x.device).cuda_stream
+    _check(lib.apic_fft2d(x.data_ptr(), x.shape[1], x.shape[0], int(inverse), C.c_void_p(stream)), "apic_fft2d")
+    return x

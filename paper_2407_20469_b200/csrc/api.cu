@@ -1,0 +1,404 @@
+// api.cu - the C ABI of libapic (include/apic.h): plan construction (host fp64 geometry ->
+// device tables + workspace) and the enqueue order of the hot path.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/apic.h"
+#include "fft_core.cuh"
+#include "plan.hpp"
+
+using namespace apic;
+
+namespace {
+
+thread_local std::string g_cuda_err;
+thread_local std::string g_plan_err;
+
+bool cuda_ok(cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return true;
+  g_cuda_err = std::string(what) + ": " + cudaGetErrorString(e);
+  return false;
+}
+
+}  // namespace
+
+struct apic_plan {
+  apic_params params{};
+  HostTables host;
+  DevTables dev{};
+  std::vector<DarkDev> dark;
+  Workspace ws{};
+  BatchState bs{};
+  std::vector<void*> allocs;
+  size_t table_bytes = 0, workspace_bytes = 0;
+  int launches = 0;
+  int32_t* h_live_count = nullptr;   // pinned
+  // staging buffers of apic_reconstruct_host (grow-only)
+  float *st_int = nullptr, *st_field = nullptr, *st_zern = nullptr, *st_pupil = nullptr;
+  int32_t* st_status = nullptr;
+  int st_batch = 0;
+  bool st_has_pupil = false;
+
+  template <class T>
+  bool dalloc(T** p, size_t count, bool table) {
+    void* q = nullptr;
+    const size_t bytes = (count ? count : 1) * sizeof(T);
+    if (!cuda_ok(cudaMalloc(&q, bytes), "cudaMalloc")) return false;
+    allocs.push_back(q);
+    (table ? table_bytes : workspace_bytes) += bytes;
+    *p = static_cast<T*>(q);
+    return true;
+  }
+  template <class T>
+  bool upload(const T** p, const std::vector<T>& v) {
+    T* q = nullptr;
+    if (!dalloc(&q, v.size(), true)) return false;
+    if (!v.empty() && !cuda_ok(cudaMemcpy(q, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice), "cudaMemcpy"))
+      return false;
+    *p = q;
+    return true;
+  }
+};
+
+static void fill_info(const HostTables& h, apic_plan_info_t* info) {
+  std::memset(info, 0, sizeof *info);
+  info->tile_n = h.n; info->upsample = h.u; info->out_n = h.n * h.u;
+  info->n_bright = h.nb; info->n_dark = h.nd; info->n_zernike = h.nz;
+  info->n_pairs = h.n_pairs;
+  info->n_rows = int(h.row_src.size() / 2);
+  info->n_grad_rows = int(h.grad_rows.size() / 2);
+  info->n_union = int(h.union_f.size());
+  info->n_known = h.n_known;
+  info->n_dark_used = int(h.dark.size());
+  for (const DarkLed& L : h.dark) {
+    info->max_unknown = std::max(info->max_unknown, L.n_unknown);
+    info->max_equations = std::max(info->max_equations, L.n_eq);
+  }
+  info->radius_bins = h.radius;
+}
+
+extern "C" {
+
+void apic_params_default(apic_params* p) {
+  std::memset(p, 0, sizeof *p);
+  p->upsample = 2;
+  p->kk_pad = 1;
+  p->refine_iters = 3;
+  p->df_iters = 48;
+  p->df_tol = 1e-6f;
+  p->intensity_floor = 1e-6f;
+  p->bg_mode = 0;
+  p->bg_threshold = 0.f;
+  p->max_batch = 64;
+  p->chunk_tiles = 0;
+}
+
+const char* apic_strerror(int err) {
+  switch (err) {
+    case APIC_OK: return "ok";
+    case APIC_EINVAL: return g_plan_err.empty() ? "invalid parameter" : g_plan_err.c_str();
+    case APIC_ECUDA: return "CUDA runtime error (see apic_last_cuda_error)";
+    case APIC_ENOMEM: return "out of memory";
+    case APIC_EBATCH: return "batch outside 1..max_batch";
+  }
+  return "unknown error";
+}
+
+const char* apic_last_cuda_error(void) { return g_cuda_err.c_str(); }
+const char* apic_version(void) { return "libapic 0.1 (sm_100a)"; }
+
+int apic_geometry_info(const apic_params* p, apic_plan_info_t* info, int* led, int* n_unknown, int* n_equations,
+                       int cap) {
+  if (!p || !info) return APIC_EINVAL;
+  HostTables h;
+  std::string err;
+  if (!build_geometry(*p, h, err)) { g_plan_err = err; return APIC_EINVAL; }
+  fill_info(h, info);
+  for (int k = 0; k < int(h.dark.size()) && k < cap; ++k) {
+    if (led) led[k] = h.dark[k].led;
+    if (n_unknown) n_unknown[k] = h.dark[k].n_unknown;
+    if (n_equations) n_equations[k] = h.dark[k].n_eq;
+  }
+  return APIC_OK;
+}
+
+int apic_plan_destroy(apic_plan* plan) {
+  if (!plan) return APIC_OK;
+  for (void* q : plan->allocs) cudaFree(q);
+  if (plan->h_live_count) cudaFreeHost(plan->h_live_count);
+  cudaFree(plan->st_int); cudaFree(plan->st_field); cudaFree(plan->st_zern); cudaFree(plan->st_pupil);
+  cudaFree(plan->st_status);
+  delete plan;
+  return APIC_OK;
+}
+
+int apic_plan_create(const apic_params* p, apic_plan** out) {
+  if (!p || !out) return APIC_EINVAL;
+  *out = nullptr;
+  int ndev = 0;
+  if (!cuda_ok(cudaGetDeviceCount(&ndev), "cudaGetDeviceCount") || ndev < 1) {
+    if (g_cuda_err.empty()) g_cuda_err = "no CUDA device";
+    return APIC_ECUDA;                                  // no CPU fallback
+  }
+  apic_plan* plan = new (std::nothrow) apic_plan;
+  if (!plan) return APIC_ENOMEM;
+  std::string err;
+  if (!build_geometry(*p, plan->host, err)) {
+    g_plan_err = err;
+    delete plan;
+    return APIC_EINVAL;
+  }
+  plan->params = *p;
+  plan->params.k_bright = nullptr; plan->params.k_dark = nullptr; plan->params.noll = nullptr;  // copied into host tables
+  const HostTables& h = plan->host;
+  DevTables& d = plan->dev;
+  const int n = h.n, nz = h.nz;
+  d.n = n; d.u = h.u; d.nb = h.nb; d.nd = h.nd; d.nz = nz; d.n_img = h.nb + h.nd;
+  bool ok = true;
+  // twiddles and output ramps, fp64 -> fp32
+  {
+    std::vector<float2> tw(n);
+    for (int m = 0; m < n; ++m) {
+      const double a = -2.0 * M_PI * m / n;
+      tw[m] = make_float2(float(std::cos(a)), float(std::sin(a)));
+    }
+    ok = ok && plan->upload(&d.tw, tw);
+    std::vector<float2> ramp(size_t(h.u) * n);
+    for (int a = 0; a < h.u; ++a)
+      for (int f = 0; f < n; ++f) {
+        const int k = f < n / 2 ? f : f - n;
+        const double ang = 2.0 * M_PI * double(k) * a / double(h.u * n);
+        ramp[size_t(a) * n + f] = make_float2(float(std::cos(ang)), float(std::sin(ang)));
+      }
+    ok = ok && plan->upload(&d.ramp, ramp);
+  }
+  ok = ok && plan->upload(&d.halfplane2, h.halfplane2);
+  d.disc_total = h.disc_off[h.nb];
+  ok = ok && plan->upload(&d.disc_zern, h.disc_zern);
+  ok = ok && plan->upload(&d.bf_col0, h.bf_col0);
+  ok = ok && plan->upload(&d.bf_ncol, h.bf_ncol);
+  ok = ok && plan->upload(&d.bf_map_off, h.bf_map_off);
+  ok = ok && plan->upload(&d.bf_map, h.bf_map);
+  d.bf_max_ncol = 0;
+  for (int v : h.bf_ncol) d.bf_max_ncol = std::max(d.bf_max_ncol, v);
+  d.n_rows = int(h.row_src.size() / 2);
+  d.n_grad = int(h.grad_rows.size() / 2);
+  ok = ok && plan->upload(&d.row_src, h.row_src);
+  ok = ok && plan->upload(&d.a_full, h.a_full);
+  ok = ok && plan->upload(&d.grad_rows, h.grad_rows);
+  d.n_union = int(h.union_f.size());
+  ok = ok && plan->upload(&d.union_f, h.union_f);
+  ok = ok && plan->upload(&d.union_off, h.union_off);
+  ok = ok && plan->upload(&d.union_src, h.union_src);
+  d.known_row0 = h.known_row0; d.known_nrow = h.known_nrow;
+  d.n_pupil = int(h.pupil_idx.size());
+  ok = ok && plan->upload(&d.pupil_idx, h.pupil_idx);
+  ok = ok && plan->upload(&d.pupil_zern, h.pupil_zern);
+  int max_eq = 1, max_unknown = 1, dot_parts = 1;
+  for (const DarkLed& L : h.dark) {
+    DarkDev q{};
+    q.n_unknown = L.n_unknown; q.n_disc = L.n_disc; q.n_eq = L.n_eq;
+    q.d_col0 = L.d_col0; q.d_ncol = L.d_ncol; q.d_row0 = L.d_row0; q.d_nrow = L.d_nrow;
+    q.u_row0 = L.u_row0; q.u_nrow = L.u_nrow;
+    q.q_col0 = L.q_col0; q.q_ncol = L.q_ncol; q.q_row0 = L.q_row0; q.q_nrow = L.q_nrow;
+    q.led = L.led;
+    ok = ok && plan->upload(&q.disc_f, L.disc_f);
+    ok = ok && plan->upload(&q.zern, L.zern);
+    ok = ok && plan->upload(&q.dmap, L.dmap);
+    ok = ok && plan->upload(&q.qmap, L.qmap);
+    plan->dark.push_back(q);
+    max_eq = std::max(max_eq, L.n_eq);
+    max_unknown = std::max(max_unknown, L.n_unknown);
+    dot_parts = std::max(dot_parts, (L.u_nrow + kLines - 1) / kLines);
+  }
+  // ---- workspace
+  Workspace& w = plan->ws;
+  const size_t nn = size_t(n) * n;
+  int chunk = p->chunk_tiles;
+  if (chunk <= 0) {
+    // darkfield CG working set per tile: T rows in use (<= 2/3 N) + p (N^2)  ~ 1.7 N^2 complex64
+    const double per_tile = 1.7 * double(nn) * sizeof(float2);
+    chunk = int(56.0e6 / per_tile);
+    chunk = std::max(8, std::min(chunk, 512));
+  }
+  chunk = std::max(1, std::min(chunk, p->max_batch));
+  w.chunk = chunk;
+  w.max_eq = max_eq; w.max_unknown = max_unknown; w.dot_parts = dot_parts;
+  const int ncol = nz + 2;
+  w.gram_entries = ncol * (ncol + 1) / 2;
+  w.gram_parts = (std::max(d.n_rows, d.n_grad) + kGramRows - 1) / kGramRows;
+  const size_t c = size_t(chunk);
+  ok = ok && plan->dalloc(&w.G, c * h.nb * nn, false);
+  ok = ok && plan->dalloc(&w.S, c * d.disc_total, false);
+  ok = ok && plan->dalloc(&w.PR, c * d.n_rows, false);
+  ok = ok && plan->dalloc(&w.gram, c * w.gram_parts * w.gram_entries, false);
+  ok = ok && plan->dalloc(&w.coef, c * nz, false);
+  ok = ok && plan->dalloc(&w.ab_fail, c, false);
+  ok = ok && plan->dalloc(&w.O, c * nn, false);
+  ok = ok && plan->dalloc(&w.T, c * nn, false);
+  ok = ok && plan->dalloc(&w.PF, c * nn, false);
+  ok = ok && plan->dalloc(&w.vec_d, c * max_eq, false);
+  ok = ok && plan->dalloc(&w.vec_x, c * max_unknown, false);
+  ok = ok && plan->dalloc(&w.vec_s, c * max_unknown, false);
+  ok = ok && plan->dalloc(&w.vec_p, c * max_unknown, false);
+  ok = ok && plan->dalloc(&w.vec_w, c * max_unknown, false);
+  ok = ok && plan->dalloc(&w.dot_part, c * dot_parts, false);
+  ok = ok && plan->dalloc(&w.cg_scal, c * 4, false);
+  ok = ok && plan->dalloc(&w.cg_done, c, false);
+  ok = ok && plan->dalloc(&w.cg_iters, c * std::max<size_t>(1, h.dark.size()), false);
+  ok = ok && plan->dalloc(&w.TOUT, c * nn * h.u, false);
+  ok = ok && plan->dalloc(&plan->bs.stats, size_t(p->max_batch) * d.n_img * 3, false);
+  ok = ok && plan->dalloc(&plan->bs.live, size_t(p->max_batch), false);
+  ok = ok && plan->dalloc(&plan->bs.live_count, 1, false);
+  ok = ok && cuda_ok(cudaMallocHost(reinterpret_cast<void**>(&plan->h_live_count), sizeof(int32_t)), "cudaMallocHost");
+  if (ok) ok = cuda_ok(cudaMemset(w.cg_iters, 0, c * std::max<size_t>(1, h.dark.size()) * sizeof(int32_t)), "cudaMemset");
+  if (!ok) {
+    const bool oom = g_cuda_err.find("out of memory") != std::string::npos;
+    apic_plan_destroy(plan);
+    return oom ? APIC_ENOMEM : APIC_ECUDA;
+  }
+  *out = plan;
+  return APIC_OK;
+}
+
+int apic_plan_info(const apic_plan* plan, apic_plan_info_t* info) {
+  if (!plan || !info) return APIC_EINVAL;
+  fill_info(plan->host, info);
+  info->chunk_tiles = plan->ws.chunk;
+  info->table_bytes = plan->table_bytes;
+  info->workspace_bytes = plan->workspace_bytes;
+  return APIC_OK;
+}
+
+int apic_plan_dark_sets(const apic_plan* plan, int* led, int* n_unknown, int* n_equations) {
+  if (!plan) return APIC_EINVAL;
+  for (size_t k = 0; k < plan->host.dark.size(); ++k) {
+    if (led) led[k] = plan->host.dark[k].led;
+    if (n_unknown) n_unknown[k] = plan->host.dark[k].n_unknown;
+    if (n_equations) n_equations[k] = plan->host.dark[k].n_eq;
+  }
+  return APIC_OK;
+}
+
+int apic_reconstruct(apic_plan* plan, const float* d_intensity, int batch, float* d_field, float* d_zernike,
+                     float* d_pupil, int32_t* d_status, void* cuda_stream) {
+  if (!plan || !d_intensity || !d_field || !d_zernike || !d_status) return APIC_EINVAL;
+  if (batch < 1 || batch > plan->params.max_batch) return APIC_EBATCH;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  const DevTables& t = plan->dev;
+  const Workspace& w = plan->ws;
+  const apic_params& p = plan->params;
+  plan->launches = 0;
+  cudaGetLastError();
+  // S0: statistics, status, list of tiles to reconstruct
+  launch_image_stats(t, d_intensity, batch, plan->bs.stats, s, &plan->launches);
+  launch_tile_status(t, plan->bs.stats, batch, p.bg_mode, p.bg_threshold, d_status, plan->bs.live,
+                     plan->bs.live_count, s, &plan->launches);
+  launch_zero_dead(t, d_status, batch, d_field, d_zernike, d_pupil, s, &plan->launches);
+  if (d_pupil) cudaMemsetAsync(d_pupil, 0, size_t(batch) * t.n * t.n * sizeof(float2), s);
+  int n_live = batch;
+  if (p.bg_mode != 0) {
+    cudaMemcpyAsync(plan->h_live_count, plan->bs.live_count, sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+    if (!cuda_ok(cudaStreamSynchronize(s), "background pass")) return APIC_ECUDA;
+    n_live = *plan->h_live_count;
+  }
+  const int n_dark_used = int(plan->dark.size());
+  for (int c0 = 0; c0 < n_live; c0 += w.chunk) {
+    LaunchCtx c{s, &plan->launches, plan->bs.live, plan->bs.live_count, c0, std::min(w.chunk, n_live - c0)};
+    launch_kk(t, w, c, d_intensity, plan->bs.stats, p.intensity_floor);                       // S1-S5
+    launch_aberration(t, w, c, p.refine_iters, d_zernike, d_status);                          // S6
+    launch_stitch(t, w, c);                                                                   // S7
+    for (int k = 0; k < n_dark_used; ++k)                                                     // S8-S10
+      launch_darkfield_led(t, plan->dark[k], k, std::max(1, n_dark_used), w, c, d_intensity, p.df_iters, p.df_tol);
+    launch_output(t, w, c, d_field, d_pupil);                                                 // S10
+  }
+  if (!cuda_ok(cudaGetLastError(), "apic_reconstruct launch")) return APIC_ECUDA;
+  return APIC_OK;
+}
+
+int apic_reconstruct_host(apic_plan* plan, const float* h_intensity, int batch, float* h_field, float* h_zernike,
+                          float* h_pupil, int32_t* h_status, void* cuda_stream) {
+  if (!plan || !h_intensity || !h_field || !h_zernike || !h_status) return APIC_EINVAL;
+  if (batch < 1 || batch > plan->params.max_batch) return APIC_EBATCH;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  const DevTables& t = plan->dev;
+  const size_t nn = size_t(t.n) * t.n, on = size_t(t.n) * t.u;
+  const size_t b_int = size_t(batch) * t.n_img * nn * sizeof(float), b_field = size_t(batch) * on * on * 2 * sizeof(float);
+  const size_t b_zern = size_t(batch) * t.nz * sizeof(float), b_pupil = size_t(batch) * nn * 2 * sizeof(float);
+  if (batch > plan->st_batch || (h_pupil && !plan->st_has_pupil)) {
+    cudaFree(plan->st_int); cudaFree(plan->st_field); cudaFree(plan->st_zern); cudaFree(plan->st_pupil);
+    cudaFree(plan->st_status);
+    plan->st_int = plan->st_field = plan->st_zern = plan->st_pupil = nullptr;
+    plan->st_status = nullptr;
+    plan->st_batch = 0;
+    bool ok = cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->st_int), b_int), "cudaMalloc staging") &&
+              cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->st_field), b_field), "cudaMalloc staging") &&
+              cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->st_zern), b_zern), "cudaMalloc staging") &&
+              cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->st_status), size_t(batch) * sizeof(int32_t)), "cudaMalloc staging");
+    if (ok && h_pupil) ok = cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->st_pupil), b_pupil), "cudaMalloc staging");
+    if (!ok) return APIC_ENOMEM;
+    plan->st_batch = batch;
+    plan->st_has_pupil = h_pupil != nullptr;
+  }
+  if (!cuda_ok(cudaMemcpyAsync(plan->st_int, h_intensity, b_int, cudaMemcpyHostToDevice, s), "H2D")) return APIC_ECUDA;
+  const int rc = apic_reconstruct(plan, plan->st_int, batch, plan->st_field, plan->st_zern,
+                                  h_pupil ? plan->st_pupil : nullptr, plan->st_status, s);
+  if (rc != APIC_OK) return rc;
+  cudaMemcpyAsync(h_field, plan->st_field, b_field, cudaMemcpyDeviceToHost, s);
+  cudaMemcpyAsync(h_zernike, plan->st_zern, b_zern, cudaMemcpyDeviceToHost, s);
+  if (h_pupil) cudaMemcpyAsync(h_pupil, plan->st_pupil, b_pupil, cudaMemcpyDeviceToHost, s);
+  cudaMemcpyAsync(h_status, plan->st_status, size_t(batch) * sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+  if (!cuda_ok(cudaStreamSynchronize(s), "apic_reconstruct_host")) return APIC_ECUDA;
+  return APIC_OK;
+}
+
+int apic_debug_buffer(const apic_plan* plan, int which, void** d_ptr, size_t* bytes_per_tile) {
+  if (!plan || !d_ptr || !bytes_per_tile) return APIC_EINVAL;
+  const DevTables& t = plan->dev;
+  switch (which) {
+    case APIC_DBG_SUBSPECTRA:
+      *d_ptr = plan->ws.S; *bytes_per_tile = size_t(t.disc_total) * sizeof(float2); return APIC_OK;
+    case APIC_DBG_OBJECT_SPECTRUM:
+      *d_ptr = plan->ws.O; *bytes_per_tile = size_t(t.n) * t.n * sizeof(float2); return APIC_OK;
+    case APIC_DBG_DF_ITERS:
+      *d_ptr = plan->ws.cg_iters; *bytes_per_tile = std::max<size_t>(1, plan->dark.size()) * sizeof(int32_t); return APIC_OK;
+  }
+  return APIC_EINVAL;
+}
+
+int apic_debug_copy(const apic_plan* plan, int which, void* d_dst, int tiles, void* cuda_stream) {
+  void* src = nullptr;
+  size_t bytes = 0;
+  const int rc = apic_debug_buffer(plan, which, &src, &bytes);
+  if (rc != APIC_OK) return rc;
+  if (!d_dst || tiles < 1 || tiles > plan->ws.chunk) return APIC_EINVAL;
+  if (!cuda_ok(cudaMemcpyAsync(d_dst, src, bytes * tiles, cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(cuda_stream)),
+               "apic_debug_copy"))
+    return APIC_ECUDA;
+  return APIC_OK;
+}
+
+int apic_fft2d(float* d_data, int n, int batch, int inverse, void* cuda_stream) {
+  if (!d_data || batch < 1 || !(n == 64 || n == 128 || n == 256 || n == 512)) return APIC_EINVAL;
+  static float2* tw_cache[4] = {nullptr, nullptr, nullptr, nullptr};
+  const int slot = n == 64 ? 0 : n == 128 ? 1 : n == 256 ? 2 : 3;
+  if (!tw_cache[slot]) {
+    std::vector<float2> tw(n);
+    for (int m = 0; m < n; ++m) {
+      const double a = -2.0 * M_PI * m / n;
+      tw[m] = make_float2(float(std::cos(a)), float(std::sin(a)));
+    }
+    if (!cuda_ok(cudaMalloc(reinterpret_cast<void**>(&tw_cache[slot]), n * sizeof(float2)), "cudaMalloc")) return APIC_ECUDA;
+    if (!cuda_ok(cudaMemcpy(tw_cache[slot], tw.data(), n * sizeof(float2), cudaMemcpyHostToDevice), "cudaMemcpy")) return APIC_ECUDA;
+  }
+  launch_fft2d(reinterpret_cast<float2*>(d_data), n, batch, inverse != 0, tw_cache[slot], static_cast<cudaStream_t>(cuda_stream));
+  if (!cuda_ok(cudaGetLastError(), "apic_fft2d")) return APIC_ECUDA;
+  return APIC_OK;
+}
+
+int apic_last_launch_count(const apic_plan* plan) { return plan ? plan->launches : 0; }
+
+}  // extern "C"

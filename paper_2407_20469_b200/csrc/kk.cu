@@ -1,0 +1,315 @@
+// kk.cu - S0 image statistics / tile status and S1-S5 Kramers-Kronig field retrieval.
+//
+// S1-S5 (Eq. 4-7; readings R5-R7 in DESIGN.md): for each NA-matching image
+//   l = log max(I, floor*mean I);  L = F(l);  G = w .* L (half-plane weights of Eq. 5);
+//   s = exp(F^-1 G);  S_hat = F(s)/N^2 kept on the disc D_i only.
+// Four strip kernels per image, every 1-D transform done in shared memory (fft_core.cuh):
+//   kk_log_rowfft : log + row FFT              [y][x]  -> [y][kx]
+//   kk_col_mask   : column FFT, w, column IFFT [y][kx] -> [ky][kx] -> [y][kx]
+//   kk_row_exp    : row IFFT, exp, row FFT     [y][kx] -> [y][x]   -> [y][kx]
+//   kk_col_gather : column FFT on the disc's columns only, gather D_i
+#include "fft_core.cuh"
+#include "plan.hpp"
+
+namespace apic {
+
+// ---------------------------------------------------------------------------------- S0 statistics
+// one CTA per (image, tile): sum, sum of squares and non-finite count of the image
+__global__ void __launch_bounds__(256) image_stats_kernel(const float* __restrict__ d_int, int npix, int n_img,
+                                                          double* __restrict__ stats) {
+  const int img = blockIdx.x, tile = blockIdx.y;
+  const float4* p = reinterpret_cast<const float4*>(d_int + (size_t(tile) * n_img + img) * npix);
+  float s = 0.f, q = 0.f;
+  int bad = 0;
+  for (int i = threadIdx.x; i < npix / 4; i += 256) {
+    float4 v = __ldg(&p[i]);
+    bad += !isfinite(v.x) + !isfinite(v.y) + !isfinite(v.z) + !isfinite(v.w);
+    s += (v.x + v.y) + (v.z + v.w);
+    q += (v.x * v.x + v.y * v.y) + (v.z * v.z + v.w * v.w);
+  }
+  __shared__ double sh[3][256];
+  sh[0][threadIdx.x] = s;
+  sh[1][threadIdx.x] = q;
+  sh[2][threadIdx.x] = bad;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (threadIdx.x < o) {
+      sh[0][threadIdx.x] += sh[0][threadIdx.x + o];
+      sh[1][threadIdx.x] += sh[1][threadIdx.x + o];
+      sh[2][threadIdx.x] += sh[2][threadIdx.x + o];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x < 3) stats[(size_t(tile) * n_img + img) * 3 + threadIdx.x] = sh[threadIdx.x][0];
+}
+
+void launch_image_stats(const DevTables& t, const float* d_int, int batch, double* stats, cudaStream_t s,
+                        int* launches) {
+  dim3 grid(t.n_img, batch);
+  image_stats_kernel<<<grid, 256, 0, s>>>(d_int, t.n * t.n, t.n_img, stats);
+  ++*launches;
+}
+
+// one warp: per-tile status (O1, BASELINE.json item 5, R18) and the ordered list of
+// tiles to reconstruct
+__global__ void tile_status_kernel(const double* __restrict__ stats, int batch, int n_img, int nb, int npix,
+                                   int bg_mode, float bg_thr, int32_t* __restrict__ status,
+                                   int32_t* __restrict__ live, int32_t* __restrict__ live_count) {
+  const int lane = threadIdx.x;
+  int count = 0;
+  for (int base = 0; base < batch; base += 32) {
+    const int tile = base + lane;
+    int st = -1;
+    if (tile < batch) {
+      const double* p = stats + size_t(tile) * n_img * 3;
+      double bad = 0, sum = 0, sq = 0;
+      for (int i = 0; i < n_img; ++i) bad += p[3 * i + 2];
+      for (int i = 0; i < nb; ++i) { sum += p[3 * i]; sq += p[3 * i + 1]; }
+      const double cnt = double(nb) * npix;
+      const double mean = sum / cnt;
+      st = 0;
+      if (bad > 0) st = 2;
+      else if (bg_mode == 1 && mean >= double(bg_thr)) st = 1;
+      else if (bg_mode == 2 && (sq / cnt - mean * mean) / (mean * mean) <= double(bg_thr)) st = 1;
+      status[tile] = st;
+    }
+    const unsigned m = __ballot_sync(0xffffffffu, st == 0);
+    if (st == 0) live[count + __popc(m & ((1u << lane) - 1u))] = tile;
+    count += __popc(m);
+  }
+  if (lane == 0) *live_count = count;
+}
+
+void launch_tile_status(const DevTables& t, const double* stats, int batch, int bg_mode, float bg_thr,
+                        int32_t* status, int32_t* live, int32_t* live_count, cudaStream_t s, int* launches) {
+  tile_status_kernel<<<1, 32, 0, s>>>(stats, batch, t.n_img, t.nb, t.n * t.n, bg_mode, bg_thr, status, live,
+                                      live_count);
+  ++*launches;
+}
+
+// background / bad-input tiles: outputs are zero
+__global__ void __launch_bounds__(256) zero_dead_kernel(const int32_t* __restrict__ status, size_t field_f4,
+                                                        int nz, size_t pupil_f4, float4* __restrict__ field,
+                                                        float* __restrict__ zern, float4* __restrict__ pupil) {
+  const int tile = blockIdx.y;
+  const int st = status[tile];
+  if (st != 1 && st != 2) return;
+  const float4 z = make_float4(0.f, 0.f, 0.f, 0.f);
+  const size_t stride = size_t(gridDim.x) * 256, t0 = size_t(blockIdx.x) * 256 + threadIdx.x;
+  for (size_t i = t0; i < field_f4; i += stride) field[size_t(tile) * field_f4 + i] = z;
+  if (pupil)
+    for (size_t i = t0; i < pupil_f4; i += stride) pupil[size_t(tile) * pupil_f4 + i] = z;
+  if (blockIdx.x == 0 && threadIdx.x < nz) zern[size_t(tile) * nz + threadIdx.x] = 0.f;
+}
+
+void launch_zero_dead(const DevTables& t, const int32_t* status, int batch, float* field, float* zern,
+                      float* pupil, cudaStream_t s, int* launches) {
+  const size_t on = size_t(t.n) * t.u;
+  dim3 grid(32, batch);
+  zero_dead_kernel<<<grid, 256, 0, s>>>(status, on * on * 2 / 4, t.nz, size_t(t.n) * t.n * 2 / 4,
+                                        reinterpret_cast<float4*>(field), zern, reinterpret_cast<float4*>(pupil));
+  ++*launches;
+}
+
+// ---------------------------------------------------------------------------------- S1-S2
+template <int N>
+__global__ void __launch_bounds__(FftCfg<N>::THREADS)
+kk_log_rowfft(DevTables t, const float* __restrict__ d_int, const double* __restrict__ stats, float floor_rel,
+              float2* __restrict__ G, const int32_t* __restrict__ live, const int32_t* __restrict__ live_count,
+              int chunk0) {
+  extern __shared__ float2 sm[];
+  const int slot = blockIdx.z, led = blockIdx.y, row0 = blockIdx.x * kLines;
+  const int tile = resolve_tile_idx(live, live_count, chunk0, slot);
+  if (tile < 0) return;
+  const float* img = d_int + (size_t(tile) * t.n_img + led) * (N * N);
+  const float mean = float(stats[(size_t(tile) * t.n_img + led) * 3] / double(N * N));
+  const float lo = floor_rel * mean;                                   // R6
+  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
+    const int l = idx / N, e = idx % N;
+    const float v = __ldg(&img[(row0 + l) * N + e]);
+    strip_at<N>(sm, l, e) = make_float2(logf(fmaxf(v, lo)), 0.f);     // Re of Eq. 4
+  }
+  __syncthreads();
+  fft_lines<N, false>(sm, t.tw);
+  float2* g = G + (size_t(slot) * t.nb + led) * (N * N);
+  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
+    const int l = idx / N, e = idx % N;
+    g[(row0 + l) * N + e] = strip_at<N>(sm, l, e);
+  }
+}
+
+// ---------------------------------------------------------------------------------- S2-S4
+template <int N>
+__global__ void __launch_bounds__(FftCfg<N>::THREADS)
+kk_col_mask(DevTables t, float2* __restrict__ G, const int32_t* __restrict__ live_count, int chunk0) {
+  extern __shared__ float2 sm[];
+  const int slot = blockIdx.z, led = blockIdx.y, x0 = blockIdx.x * kLines;
+  if (chunk0 + slot >= *live_count) return;
+  float2* g = G + (size_t(slot) * t.nb + led) * (N * N);
+  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
+    const int l = idx % kLines, e = idx / kLines;
+    strip_at<N>(sm, l, e) = g[e * N + x0 + l];
+  }
+  __syncthreads();
+  fft_lines<N, false>(sm, t.tw);
+  const uint8_t* w2 = t.halfplane2 + size_t(led) * (N * N);
+  const float scale = 0.5f / float(N * N);                              // w = w2/2, and the 1/N^2 of F^-1
+  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
+    const int l = idx % kLines, e = idx / kLines;                       // e = fy, column fx = x0 + l
+    const float w = float(w2[e * N + x0 + l]) * scale;                  // Eq. 5
+    float2& v = strip_at<N>(sm, l, e);
+    v = cscale(v, w);
+  }
+  __syncthreads();
+  fft_lines<N, true>(sm, t.tw);
+  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
+    const int l = idx % kLines, e = idx / kLines;
+    g[e * N + x0 + l] = strip_at<N>(sm, l, e);
+  }
+}
+
+// ---------------------------------------------------------------------------------- S4-S5
+template <int N>
+__global__ void __launch_bounds__(FftCfg<N>::THREADS)
+kk_row_exp(DevTables t, float2* __restrict__ G, const int32_t* __restrict__ live_count, int chunk0) {
+  extern __shared__ float2 sm[];
+  const int slot = blockIdx.z, led = blockIdx.y, row0 = blockIdx.x * kLines;
+  if (chunk0 + slot >= *live_count) return;
+  float2* g = G + (size_t(slot) * t.nb + led) * (N * N);
+  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
+    const int l = idx / N, e = idx % N;
+    strip_at<N>(sm, l, e) = g[(row0 + l) * N + e];
+  }
+  __syncthreads();
+  fft_lines<N, true>(sm, t.tw);
+  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
+    const int l = idx / N, e = idx % N;
+    float2& v = strip_at<N>(sm, l, e);
+    const float a = expf(v.x);                                          // Eq. 6
+    float sn, cs;
+    sincosf(v.y, &sn, &cs);
+    v = make_float2(a * cs, a * sn);
+  }
+  __syncthreads();
+  fft_lines<N, false>(sm, t.tw);
+  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
+    const int l = idx / N, e = idx % N;
+    g[(row0 + l) * N + e] = strip_at<N>(sm, l, e);
+  }
+}
+
+// ---------------------------------------------------------------------------------- S5 (Eq. 7)
+template <int N>
+__global__ void __launch_bounds__(FftCfg<N>::THREADS)
+kk_col_gather(DevTables t, const float2* __restrict__ G, float2* __restrict__ S,
+              const int32_t* __restrict__ live_count, int chunk0) {
+  extern __shared__ float2 sm[];
+  const int slot = blockIdx.z, led = blockIdx.y, c0 = blockIdx.x * kLines;
+  if (chunk0 + slot >= *live_count) return;
+  const int ncol = t.bf_ncol[led];
+  if (c0 >= ncol) return;
+  const int col0 = t.bf_col0[led];
+  const float2* g = G + (size_t(slot) * t.nb + led) * (N * N);
+  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
+    const int l = idx % kLines, e = idx / kLines;
+    float2 v = make_float2(0.f, 0.f);
+    if (c0 + l < ncol) v = g[e * N + ((col0 + c0 + l + N) & (N - 1))];
+    strip_at<N>(sm, l, e) = v;
+  }
+  __syncthreads();
+  fft_lines<N, false>(sm, t.tw);
+  const int32_t* map = t.bf_map + t.bf_map_off[led];
+  float2* s = S + size_t(slot) * t.disc_total;
+  const float scale = 1.f / float(N * N);
+  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
+    const int l = idx % kLines, e = idx / kLines;
+    if (c0 + l >= ncol) continue;
+    const int ent = map[e * ncol + c0 + l];
+    if (ent >= 0) s[ent] = cscale(strip_at<N>(sm, l, e), scale);
+  }
+}
+
+template <int N>
+static void launch_kk_n(const DevTables& t, const Workspace& w, const LaunchCtx& c, const float* d_int,
+                        const double* stats, float floor_rel) {
+  constexpr int TH = FftCfg<N>::THREADS;
+  constexpr size_t SM = strip_smem_bytes(N);
+  static bool attr = false;
+  if (!attr) {
+    cudaFuncSetAttribute(kk_log_rowfft<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
+    cudaFuncSetAttribute(kk_col_mask<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
+    cudaFuncSetAttribute(kk_row_exp<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
+    cudaFuncSetAttribute(kk_col_gather<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
+    attr = true;
+  }
+  dim3 grid(N / kLines, t.nb, c.chunk_tiles);
+  kk_log_rowfft<N><<<grid, TH, SM, c.stream>>>(t, d_int, stats, floor_rel, w.G, c.live, c.live_count, c.chunk0);
+  kk_col_mask<N><<<grid, TH, SM, c.stream>>>(t, w.G, c.live_count, c.chunk0);
+  kk_row_exp<N><<<grid, TH, SM, c.stream>>>(t, w.G, c.live_count, c.chunk0);
+  dim3 grid4((t.bf_max_ncol + kLines - 1) / kLines, t.nb, c.chunk_tiles);
+  kk_col_gather<N><<<grid4, TH, SM, c.stream>>>(t, w.G, w.S, c.live_count, c.chunk0);
+  *c.launches += 4;
+}
+
+void launch_kk(const DevTables& t, const Workspace& w, const LaunchCtx& c, const float* d_int, const double* stats,
+               float floor_rel) {
+  switch (t.n) {
+    case 64: launch_kk_n<64>(t, w, c, d_int, stats, floor_rel); break;
+    case 128: launch_kk_n<128>(t, w, c, d_int, stats, floor_rel); break;
+    case 256: launch_kk_n<256>(t, w, c, d_int, stats, floor_rel); break;
+    case 512: launch_kk_n<512>(t, w, c, d_int, stats, floor_rel); break;
+  }
+}
+
+// ---------------------------------------------------------------------------------- plain 2-D FFT
+template <int N, bool INV, bool COLS>
+__global__ void __launch_bounds__(FftCfg<N>::THREADS) fft_pass_kernel(float2* __restrict__ d, const float2* __restrict__ tw) {
+  extern __shared__ float2 sm[];
+  float2* g = d + size_t(blockIdx.y) * (N * N);
+  const int s0 = blockIdx.x * kLines;
+  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
+    if (COLS) { const int l = idx % kLines, e = idx / kLines; strip_at<N>(sm, l, e) = g[e * N + s0 + l]; }
+    else      { const int l = idx / N, e = idx % N;           strip_at<N>(sm, l, e) = g[(s0 + l) * N + e]; }
+  }
+  __syncthreads();
+  fft_lines<N, INV>(sm, tw);
+  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
+    if (COLS) { const int l = idx % kLines, e = idx / kLines; g[e * N + s0 + l] = strip_at<N>(sm, l, e); }
+    else      { const int l = idx / N, e = idx % N;           g[(s0 + l) * N + e] = strip_at<N>(sm, l, e); }
+  }
+}
+
+template <int N>
+static int fft2d_n(float2* d, int batch, bool inverse, const float2* tw, cudaStream_t s) {
+  constexpr int TH = FftCfg<N>::THREADS;
+  constexpr size_t SM = strip_smem_bytes(N);
+  cudaFuncSetAttribute(fft_pass_kernel<N, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
+  cudaFuncSetAttribute(fft_pass_kernel<N, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
+  cudaFuncSetAttribute(fft_pass_kernel<N, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
+  cudaFuncSetAttribute(fft_pass_kernel<N, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
+  for (int b0 = 0; b0 < batch; b0 += 32768) {
+    const int nb = batch - b0 < 32768 ? batch - b0 : 32768;
+    dim3 grid(N / kLines, nb);
+    float2* p = d + size_t(b0) * (N * N);
+    if (inverse) {
+      fft_pass_kernel<N, true, false><<<grid, TH, SM, s>>>(p, tw);
+      fft_pass_kernel<N, true, true><<<grid, TH, SM, s>>>(p, tw);
+    } else {
+      fft_pass_kernel<N, false, false><<<grid, TH, SM, s>>>(p, tw);
+      fft_pass_kernel<N, false, true><<<grid, TH, SM, s>>>(p, tw);
+    }
+  }
+  return 0;
+}
+
+int launch_fft2d(float2* d, int n, int batch, bool inverse, const float2* tw, cudaStream_t s) {
+  switch (n) {
+    case 64: return fft2d_n<64>(d, batch, inverse, tw, s);
+    case 128: return fft2d_n<128>(d, batch, inverse, tw, s);
+    case 256: return fft2d_n<256>(d, batch, inverse, tw, s);
+    case 512: return fft2d_n<512>(d, batch, inverse, tw, s);
+  }
+  return -1;
+}
+
+}  // namespace apic

@@ -1,0 +1,133 @@
+// plan.hpp - device-side view of an apic_plan: geometry tables (read-only, identical for every
+// tile) and the per-chunk workspace.  Shared by the kernel translation units and api.cu.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "geometry.hpp"
+
+namespace apic {
+
+struct DevTables {
+  int n, u, nb, nd, nz, n_img;   // n_img = nb + nd
+  const float2* tw;              // [N] e^{-2 pi i m / N}
+  // NA-matching side
+  const uint8_t* halfplane2;     // [nb][N*N] FFT order, 2*w of Eq. 5
+  int disc_total;                // sum_i |D_i|
+  const float* disc_zern;        // [disc_total][nz]  Z_j(K+kappa_i) - Z_j(kappa_i)
+  const int32_t* bf_col0;        // [nb]
+  const int32_t* bf_ncol;        // [nb]
+  const int32_t* bf_map_off;     // [nb+1]
+  const int32_t* bf_map;         // per LED [N(fy)][ncol] -> flattened entry | -1
+  int bf_max_ncol;
+  // aberration system
+  int n_rows, n_grad;
+  const int32_t* row_src;        // [n_rows][2]
+  const float* a_full;           // [n_rows][nz]
+  const int32_t* grad_rows;      // [n_grad][2]
+  // stitching
+  int n_union;
+  const int32_t* union_f;        // [n_union]
+  const int32_t* union_off;      // [n_union+1]
+  const int32_t* union_src;
+  // output
+  int known_row0, known_nrow;    // centred ky range of the final known region
+  const float2* ramp;            // [u][N]: e^{+2 pi i k a / (uN)}, index a*N + (k mod N), k signed bin
+  int n_pupil;
+  const int32_t* pupil_idx;      // centred linear index
+  const float* pupil_zern;       // [n_pupil][nz]
+};
+
+struct DarkDev {
+  int n_unknown, n_disc, n_eq;
+  int d_col0, d_ncol, d_row0, d_nrow;   // disc bbox (centred)
+  int u_row0, u_nrow;                   // rows holding unknown bins
+  int q_col0, q_ncol, q_row0, q_nrow;   // bbox of the linear region Q
+  const int32_t* disc_f;                // [n_disc] FFT-order index (U entries first)
+  const float* zern;                    // [n_disc][nz] Z_j(K + kappa)
+  const int32_t* dmap;                  // [N(fy)][d_ncol] -> disc entry | -1
+  const int32_t* qmap;                  // [N(fy)][q_ncol] -> equation | -1
+  int led;                              // input index among the darkfield LEDs
+};
+
+constexpr int kGramRows = 512;          // rows per Gram partial (aberration kernels)
+constexpr int kMaxZern = 64;
+
+struct Workspace {
+  int chunk;               // tiles per pass
+  float2* G;               // [chunk][nb][N*N]   KK working grids
+  float2* S;               // [chunk][disc_total] sub-spectra on the discs (Eq. 7)
+  float2* PR;              // [chunk][n_rows]    p = S_i conj S_l on the overlaps (Eq. 9)
+  float* gram;             // [chunk][gram_parts][gram_entries]
+  int gram_parts, gram_entries;
+  float* coef;             // [chunk][nz]
+  int32_t* ab_fail;        // [chunk] Cholesky failure flag
+  float2* O;               // [chunk][N*N] object spectrum, FFT order
+  float2* T;               // [chunk][N*N] transform scratch
+  float2* PF;              // [chunk][N*N] p = F^-1 P_hat of the current darkfield LED
+  float2* vec_d;           // [chunk][max_eq]
+  float2* vec_x;           // [chunk][max_unknown]
+  float2* vec_s;
+  float2* vec_p;
+  float2* vec_w;
+  float* dot_part;         // [chunk][dot_parts]
+  int dot_parts;
+  float* cg_scal;          // [chunk][4]: gamma, gamma0, -, -
+  int32_t* cg_done;        // [chunk]
+  int32_t* cg_iters;       // [chunk][n_dark_used]
+  float2* TOUT;            // [chunk][N][uN]
+  int max_eq, max_unknown;
+};
+
+// Batch-level state
+struct BatchState {
+  double* stats;           // [max_batch][n_img][3]: sum, sum of squares, non-finite count
+  int32_t* live;           // [max_batch] compacted list of tiles to reconstruct
+  int32_t* live_count;     // device scalar
+};
+
+// ------------------------------------------------------------------ launchers (one per kernel)
+struct LaunchCtx {
+  cudaStream_t stream;
+  int* launches;           // counter
+  const int32_t* live;     // compacted tile list
+  const int32_t* live_count;
+  int chunk0;              // first live-list position of this chunk
+  int chunk_tiles;         // grid size in tiles (CTAs beyond live_count exit)
+};
+
+// stats / status (batch-level)
+void launch_image_stats(const DevTables& t, const float* d_int, int batch, double* stats, cudaStream_t s, int* launches);
+void launch_tile_status(const DevTables& t, const double* stats, int batch, int bg_mode, float bg_thr,
+                        int32_t* status, int32_t* live, int32_t* live_count, cudaStream_t s, int* launches);
+void launch_zero_dead(const DevTables& t, const int32_t* status, int batch, float* field, float* zern,
+                      float* pupil, cudaStream_t s, int* launches);
+
+// KK (S1-S5)
+void launch_kk(const DevTables& t, const Workspace& w, const LaunchCtx& c, const float* d_int,
+               const double* stats, float floor_rel);
+// aberration (S6) + stitching (S7)
+void launch_aberration(const DevTables& t, const Workspace& w, const LaunchCtx& c, int refine_iters,
+                       float* d_zernike, int32_t* d_status);
+void launch_stitch(const DevTables& t, const Workspace& w, const LaunchCtx& c);
+// darkfield (S8-S10) for one LED
+void launch_darkfield_led(const DevTables& t, const DarkDev& L, int led_pos, int n_dark_used, const Workspace& w,
+                          const LaunchCtx& c, const float* d_int, int df_iters, float df_tol);
+// outputs
+void launch_output(const DevTables& t, const Workspace& w, const LaunchCtx& c, float* d_field, float* d_pupil);
+
+// plain batched 2-D FFT (apic_fft2d)
+int launch_fft2d(float2* d, int n, int batch, bool inverse, const float2* tw, cudaStream_t s);
+
+#ifdef __CUDACC__
+// tile handled by chunk-local slot `slot` (-1: beyond the live list)
+__device__ __forceinline__ int resolve_tile_idx(const int32_t* __restrict__ live,
+                                                const int32_t* __restrict__ live_count, int chunk0, int slot) {
+  const int pos = chunk0 + slot;
+  if (pos >= *live_count) return -1;
+  return live[pos];
+}
+#endif
+
+}  // namespace apic
