@@ -76,7 +76,7 @@ typedef struct {
                             working set stays inside the 126 MB L2                              */
 } apic_params;
 
-/* Fills *p with the defaults (kk_pad 1, refine_iters 3, df_iters 48, df_tol 1e-6, floor 1e-6,
+/* Fills *p with the defaults (kk_pad 1, refine_iters 3, df_iters 48, df_tol 1e-5, floor 1e-6,
  * bg off, max_batch 64); the caller then sets the geometry fields. */
 void apic_params_default(apic_params* p);
 
@@ -156,6 +156,17 @@ int apic_fft2d(float* d_data, int n, int batch, int inverse, void* cuda_stream);
 
 /* Number of kernels launched by the last apic_reconstruct on this plan (bench's gpu_launches). */
 int apic_last_launch_count(const apic_plan* plan);
+
+/* Per-kernel timing for bench.py's roofline line.  Between apic_profile_begin and apic_profile_end
+ * every `stride`-th launch of each kernel category made by apic_reconstruct on this plan is
+ * bracketed by CUDA events on the launching stream (at most max_samples launches in total).
+ * apic_profile_end synchronises those events and fills, per category (apic_profile_categories()
+ * entries, named by apic_profile_category_name): the summed duration of the sampled launches in
+ * ms, the number of sampled launches, and the number of all launches since apic_profile_begin. */
+int apic_profile_categories(void);
+const char* apic_profile_category_name(int cat);
+int apic_profile_begin(apic_plan* plan, int stride, int max_samples);
+int apic_profile_end(apic_plan* plan, double* ms_sum, long long* samples, long long* launches);
 
 const char* apic_strerror(int err);
 const char* apic_last_cuda_error(void);

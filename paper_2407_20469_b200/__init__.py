@@ -23,7 +23,8 @@ DBG_SUBSPECTRA, DBG_OBJECT_SPECTRUM, DBG_DF_ITERS = 0, 1, 2
 EXPORTS = ("apic_params_default", "apic_plan_create", "apic_plan_destroy", "apic_plan_info",
            "apic_geometry_info", "apic_plan_dark_sets", "apic_reconstruct", "apic_reconstruct_host",
            "apic_debug_buffer", "apic_debug_copy", "apic_fft2d", "apic_last_launch_count", "apic_strerror",
-           "apic_last_cuda_error", "apic_version")
+           "apic_last_cuda_error", "apic_version", "apic_profile_categories", "apic_profile_category_name",
+           "apic_profile_begin", "apic_profile_end")
 
 
 class ApicError(RuntimeError):
@@ -81,6 +82,11 @@ def load() -> C.CDLL:
     for name in ("apic_strerror", "apic_last_cuda_error", "apic_version"):
         getattr(lib, name).restype = C.c_char_p
     lib.apic_strerror.argtypes = [C.c_int]
+    lib.apic_profile_category_name.restype = C.c_char_p
+    lib.apic_profile_category_name.argtypes = [C.c_int]
+    lib.apic_profile_begin.argtypes = [C.c_void_p, C.c_int, C.c_int]
+    lib.apic_profile_end.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_longlong),
+                                     C.POINTER(C.c_longlong)]
     _lib = lib
     return lib
 
@@ -216,6 +222,16 @@ class Plan:
         if which == DBG_DF_ITERS:
             return out.view(torch.int32).view(tiles, -1)
         return out.view(torch.complex64).view(tiles, -1)
+
+    def profile_begin(self, stride: int = 1, max_samples: int = 8192):
+        _check(self._lib.apic_profile_begin(self._h, stride, max_samples), "apic_profile_begin")
+
+    def profile_end(self):
+        """{kernel: (ms summed over the sampled launches, sampled launches, all launches)}"""
+        n = self._lib.apic_profile_categories()
+        ms, sm, la = (C.c_double * n)(), (C.c_longlong * n)(), (C.c_longlong * n)()
+        _check(self._lib.apic_profile_end(self._h, ms, sm, la), "apic_profile_end")
+        return {self._lib.apic_profile_category_name(i).decode(): (ms[i], sm[i], la[i]) for i in range(n)}
 
     @property
     def last_launch_count(self) -> int:

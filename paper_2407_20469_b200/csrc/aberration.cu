@@ -189,23 +189,26 @@ void launch_aberration(const DevTables& t, const Workspace& w, const LaunchCtx& 
     attr = true;
   }
   dim3 g1((t.n_rows + 255) / 256, c.chunk_tiles);
-  ab_pair_products<<<g1, 256, 0, c.stream>>>(t, w.S, w.PR, c.live_count, c.chunk0);
+  { ProfScope ps(c, CAT_AB_PRODUCTS);
+    ab_pair_products<<<g1, 256, 0, c.stream>>>(t, w.S, w.PR, c.live_count, c.chunk0); }
   const int parts_g = (t.n_grad + kGramRows - 1) / kGramRows, parts_f = (t.n_rows + kGramRows - 1) / kGramRows;
-  ab_gram<0><<<dim3(parts_g, c.chunk_tiles), 256, sm, c.stream>>>(t, w.PR, w.coef, w.gram, parts_g, w.gram_entries,
-                                                                    c.live_count, c.chunk0);
-  ab_solve<0><<<c.chunk_tiles, 128, 0, c.stream>>>(t, w.gram, parts_g, w.gram_entries, w.coef, w.ab_fail, d_zernike,
-                                                   d_status, c.live, c.live_count, c.chunk0);
-  *c.launches += 3;
+  { ProfScope ps(c, CAT_AB_GRAM);
+    ab_gram<0><<<dim3(parts_g, c.chunk_tiles), 256, sm, c.stream>>>(t, w.PR, w.coef, w.gram, parts_g, w.gram_entries,
+                                                                      c.live_count, c.chunk0); }
+  { ProfScope ps(c, CAT_AB_SOLVE);
+    ab_solve<0><<<c.chunk_tiles, 128, 0, c.stream>>>(t, w.gram, parts_g, w.gram_entries, w.coef, w.ab_fail, d_zernike,
+                                                     d_status, c.live, c.live_count, c.chunk0); }
   for (int it = 0; it <= refine_iters; ++it) {
-    ab_gram<1><<<dim3(parts_f, c.chunk_tiles), 256, sm, c.stream>>>(t, w.PR, w.coef, w.gram, parts_f, w.gram_entries,
-                                                                      c.live_count, c.chunk0);
+    { ProfScope ps(c, CAT_AB_GRAM);
+      ab_gram<1><<<dim3(parts_f, c.chunk_tiles), 256, sm, c.stream>>>(t, w.PR, w.coef, w.gram, parts_f,
+                                                                        w.gram_entries, c.live_count, c.chunk0); }
+    ProfScope ps(c, CAT_AB_SOLVE);
     if (it < refine_iters)
       ab_solve<1><<<c.chunk_tiles, 128, 0, c.stream>>>(t, w.gram, parts_f, w.gram_entries, w.coef, w.ab_fail,
                                                        d_zernike, d_status, c.live, c.live_count, c.chunk0);
     else
       ab_solve<2><<<c.chunk_tiles, 128, 0, c.stream>>>(t, w.gram, parts_f, w.gram_entries, w.coef, w.ab_fail,
                                                        d_zernike, d_status, c.live, c.live_count, c.chunk0);
-    *c.launches += 2;
   }
 }
 
@@ -237,9 +240,9 @@ __global__ void __launch_bounds__(256) stitch_kernel(DevTables t, const float2* 
 
 void launch_stitch(const DevTables& t, const Workspace& w, const LaunchCtx& c) {
   cudaMemsetAsync(w.O, 0, size_t(c.chunk_tiles) * t.n * t.n * sizeof(float2), c.stream);
+  ProfScope ps(c, CAT_STITCH);
   stitch_kernel<<<dim3((t.n_union + 255) / 256, c.chunk_tiles), 256, 0, c.stream>>>(t, w.S, w.coef, w.O, c.live_count,
                                                                                      c.chunk0);
-  *c.launches += 1;
 }
 
 }  // namespace apic

@@ -35,6 +35,7 @@ struct apic_plan {
   std::vector<void*> allocs;
   size_t table_bytes = 0, workspace_bytes = 0;
   int launches = 0;
+  Profiler prof;
   int32_t* h_live_count = nullptr;   // pinned
   // staging buffers of apic_reconstruct_host (grow-only)
   float *st_int = nullptr, *st_field = nullptr, *st_zern = nullptr, *st_pupil = nullptr;
@@ -88,7 +89,7 @@ void apic_params_default(apic_params* p) {
   p->kk_pad = 1;
   p->refine_iters = 3;
   p->df_iters = 48;
-  p->df_tol = 1e-6f;
+  p->df_tol = 1e-5f;
   p->intensity_floor = 1e-6f;
   p->bg_mode = 0;
   p->bg_threshold = 0.f;
@@ -128,6 +129,7 @@ int apic_geometry_info(const apic_params* p, apic_plan_info_t* info, int* led, i
 int apic_plan_destroy(apic_plan* plan) {
   if (!plan) return APIC_OK;
   for (void* q : plan->allocs) cudaFree(q);
+  for (cudaEvent_t e : plan->prof.ev) cudaEventDestroy(e);
   if (plan->h_live_count) cudaFreeHost(plan->h_live_count);
   cudaFree(plan->st_int); cudaFree(plan->st_field); cudaFree(plan->st_zern); cudaFree(plan->st_pupil);
   cudaFree(plan->st_status);
@@ -294,10 +296,13 @@ int apic_reconstruct(apic_plan* plan, const float* d_intensity, int batch, float
   plan->launches = 0;
   cudaGetLastError();
   // S0: statistics, status, list of tiles to reconstruct
-  launch_image_stats(t, d_intensity, batch, plan->bs.stats, s, &plan->launches);
-  launch_tile_status(t, plan->bs.stats, batch, p.bg_mode, p.bg_threshold, d_status, plan->bs.live,
-                     plan->bs.live_count, s, &plan->launches);
-  launch_zero_dead(t, d_status, batch, d_field, d_zernike, d_pupil, s, &plan->launches);
+  {
+    LaunchCtx c{s, &plan->launches, &plan->prof, plan->bs.live, plan->bs.live_count, 0, batch};
+    launch_image_stats(t, d_intensity, batch, plan->bs.stats, c);
+    launch_tile_status(t, plan->bs.stats, batch, p.bg_mode, p.bg_threshold, d_status, plan->bs.live,
+                       plan->bs.live_count, c);
+    launch_zero_dead(t, d_status, batch, d_field, d_zernike, d_pupil, c);
+  }
   if (d_pupil) cudaMemsetAsync(d_pupil, 0, size_t(batch) * t.n * t.n * sizeof(float2), s);
   int n_live = batch;
   if (p.bg_mode != 0) {
@@ -307,7 +312,8 @@ int apic_reconstruct(apic_plan* plan, const float* d_intensity, int batch, float
   }
   const int n_dark_used = int(plan->dark.size());
   for (int c0 = 0; c0 < n_live; c0 += w.chunk) {
-    LaunchCtx c{s, &plan->launches, plan->bs.live, plan->bs.live_count, c0, std::min(w.chunk, n_live - c0)};
+    LaunchCtx c{s, &plan->launches, &plan->prof, plan->bs.live, plan->bs.live_count, c0,
+                std::min(w.chunk, n_live - c0)};
     launch_kk(t, w, c, d_intensity, plan->bs.stats, p.intensity_floor);                       // S1-S5
     launch_aberration(t, w, c, p.refine_iters, d_zernike, d_status);                          // S6
     launch_stitch(t, w, c);                                                                   // S7
@@ -400,5 +406,45 @@ int apic_fft2d(float* d_data, int n, int batch, int inverse, void* cuda_stream) 
 }
 
 int apic_last_launch_count(const apic_plan* plan) { return plan ? plan->launches : 0; }
+
+static const char* kCatNames[CAT_COUNT] = {
+    "stats_status", "kk_log_rowfft", "kk_col_mask", "kk_row_exp", "kk_col_gather", "ab_pair_products", "ab_gram",
+    "ab_solve", "stitch", "df_build_p_rows", "df_cols_p", "df_rows_rhs", "df_rows_q", "df_cols_mul",
+    "df_rows_u_scatter", "df_rows_u_gather", "df_cg_vector", "df_extend", "out_rows", "out_cols", "pupil"};
+
+int apic_profile_categories(void) { return CAT_COUNT; }
+const char* apic_profile_category_name(int cat) { return (cat >= 0 && cat < CAT_COUNT) ? kCatNames[cat] : ""; }
+
+int apic_profile_begin(apic_plan* plan, int stride, int max_samples) {
+  if (!plan || stride < 1 || max_samples < 1) return APIC_EINVAL;
+  Profiler& pr = plan->prof;
+  while (int(pr.ev.size()) < 2 * max_samples) {
+    cudaEvent_t e;
+    if (!cuda_ok(cudaEventCreate(&e), "cudaEventCreate")) return APIC_ECUDA;
+    pr.ev.push_back(e);
+  }
+  pr.cat.assign(pr.ev.size() / 2, 0);
+  pr.used = 0;
+  pr.stride = stride;
+  for (long long& v : pr.launches) v = 0;
+  pr.on = true;
+  return APIC_OK;
+}
+
+int apic_profile_end(apic_plan* plan, double* ms_sum, long long* samples, long long* launches) {
+  if (!plan || !ms_sum || !samples || !launches) return APIC_EINVAL;
+  Profiler& pr = plan->prof;
+  pr.on = false;
+  for (int c = 0; c < CAT_COUNT; ++c) { ms_sum[c] = 0; samples[c] = 0; launches[c] = pr.launches[c]; }
+  for (int i = 0; i < pr.used; ++i) {
+    if (!cuda_ok(cudaEventSynchronize(pr.ev[2 * i + 1]), "cudaEventSynchronize")) return APIC_ECUDA;
+    float ms = 0.f;
+    if (!cuda_ok(cudaEventElapsedTime(&ms, pr.ev[2 * i], pr.ev[2 * i + 1]), "cudaEventElapsedTime")) return APIC_ECUDA;
+    ms_sum[pr.cat[i]] += ms;
+    samples[pr.cat[i]] += 1;
+  }
+  pr.used = 0;
+  return APIC_OK;
+}
 
 }  // extern "C"

@@ -419,36 +419,49 @@ static void darkfield_led_n(const DevTables& t, const DarkDev& L, int led_pos, i
   const dim3 g_d(strips(L.d_nrow), B), g_q(strips(L.q_nrow), B), g_u(strips(L.u_nrow), B), g_c(N / kLines, B);
   const int n_parts = strips(L.u_nrow);
 
-  df_build_p_rows<N><<<g_d, TH, SM, s>>>(t, L, w.O, w.coef, w.T, c.live_count, c.chunk0);
-  df_cols_p<N><<<g_c, TH, SM, s>>>(t, L, d_int, w.T, w.PF, c.live, c.live_count, c.chunk0);
-  df_rows_rhs<N><<<g_q, TH, SM, s>>>(t, L, w.T, w.vec_d, w.max_eq, c.live_count, c.chunk0);
+#define APIC_LAUNCH(cat, ...) do { ProfScope ps_(c, cat); __VA_ARGS__; } while (0)
+  APIC_LAUNCH(CAT_DF_BUILD_P_ROWS,
+              (df_build_p_rows<N><<<g_d, TH, SM, s>>>(t, L, w.O, w.coef, w.T, c.live_count, c.chunk0)));
+  APIC_LAUNCH(CAT_DF_COLS_P,
+              (df_cols_p<N><<<g_c, TH, SM, s>>>(t, L, d_int, w.T, w.PF, c.live, c.live_count, c.chunk0)));
+  APIC_LAUNCH(CAT_DF_ROWS_RHS,
+              (df_rows_rhs<N><<<g_q, TH, SM, s>>>(t, L, w.T, w.vec_d, w.max_eq, c.live_count, c.chunk0)));
   // s0 = C^H d
-  df_rows_q<N, true><<<g_q, TH, SM, s>>>(t, L, w.T, w.vec_d, w.max_eq, w.cg_done, c.live_count, c.chunk0);
-  df_cols_mul<N, false><<<g_c, TH, SM, s>>>(t, w.T, w.PF, L.q_row0, L.q_nrow, L.u_row0, L.u_nrow, w.cg_done, 0,
-                                            c.live_count, c.chunk0);
-  df_rows_u_gather<N><<<g_u, TH, SM, s>>>(t, L, w.T, w.vec_w, w.vec_p, w.max_unknown, w.dot_part, w.dot_parts,
-                                          w.cg_done, 0, c.live_count, c.chunk0);
-  df_cg_init<<<B, 256, 0, s>>>(L.n_unknown, w.max_unknown, w.vec_x, w.vec_s, w.vec_p, w.vec_w, w.cg_scal, w.cg_done,
-                               w.cg_iters, n_dark_used, led_pos, c.live_count, c.chunk0);
-  *c.launches += 7;
+  APIC_LAUNCH(CAT_DF_ROWS_Q, (df_rows_q<N, true><<<g_q, TH, SM, s>>>(t, L, w.T, w.vec_d, w.max_eq, w.cg_done,
+                                                                     c.live_count, c.chunk0)));
+  APIC_LAUNCH(CAT_DF_COLS_MUL,
+              (df_cols_mul<N, false><<<g_c, TH, SM, s>>>(t, w.T, w.PF, L.q_row0, L.q_nrow, L.u_row0, L.u_nrow,
+                                                         w.cg_done, 0, c.live_count, c.chunk0)));
+  APIC_LAUNCH(CAT_DF_ROWS_U_GATHER,
+              (df_rows_u_gather<N><<<g_u, TH, SM, s>>>(t, L, w.T, w.vec_w, w.vec_p, w.max_unknown, w.dot_part,
+                                                       w.dot_parts, w.cg_done, 0, c.live_count, c.chunk0)));
+  APIC_LAUNCH(CAT_DF_CG_VECTOR,
+              (df_cg_init<<<B, 256, 0, s>>>(L.n_unknown, w.max_unknown, w.vec_x, w.vec_s, w.vec_p, w.vec_w, w.cg_scal,
+                                            w.cg_done, w.cg_iters, n_dark_used, led_pos, c.live_count, c.chunk0)));
   const float tol2 = df_tol * df_tol;
   for (int it = 0; it < df_iters; ++it) {
-    df_rows_u_scatter<N><<<g_u, TH, SM, s>>>(t, L, w.T, w.vec_p, w.max_unknown, w.cg_done, c.live_count, c.chunk0);
-    df_cols_mul<N, true><<<g_c, TH, SM, s>>>(t, w.T, w.PF, L.u_row0, L.u_nrow, L.q_row0, L.q_nrow, w.cg_done, 1,
-                                             c.live_count, c.chunk0);
-    df_rows_q<N, false><<<g_q, TH, SM, s>>>(t, L, w.T, w.vec_d, w.max_eq, w.cg_done, c.live_count, c.chunk0);
-    df_cols_mul<N, false><<<g_c, TH, SM, s>>>(t, w.T, w.PF, L.q_row0, L.q_nrow, L.u_row0, L.u_nrow, w.cg_done, 1,
-                                              c.live_count, c.chunk0);
-    df_rows_u_gather<N><<<g_u, TH, SM, s>>>(t, L, w.T, w.vec_w, w.vec_p, w.max_unknown, w.dot_part, w.dot_parts,
-                                            w.cg_done, 1, c.live_count, c.chunk0);
-    df_cg_update<<<B, 256, 0, s>>>(L.n_unknown, w.max_unknown, w.vec_x, w.vec_s, w.vec_p, w.vec_w, w.dot_part,
-                                   w.dot_parts, n_parts, w.cg_scal, w.cg_done, w.cg_iters, n_dark_used, led_pos, tol2,
-                                   c.live_count, c.chunk0);
-    *c.launches += 6;
+    APIC_LAUNCH(CAT_DF_ROWS_U_SCATTER,
+                (df_rows_u_scatter<N><<<g_u, TH, SM, s>>>(t, L, w.T, w.vec_p, w.max_unknown, w.cg_done, c.live_count,
+                                                          c.chunk0)));
+    APIC_LAUNCH(CAT_DF_COLS_MUL,
+                (df_cols_mul<N, true><<<g_c, TH, SM, s>>>(t, w.T, w.PF, L.u_row0, L.u_nrow, L.q_row0, L.q_nrow,
+                                                          w.cg_done, 1, c.live_count, c.chunk0)));
+    APIC_LAUNCH(CAT_DF_ROWS_Q, (df_rows_q<N, false><<<g_q, TH, SM, s>>>(t, L, w.T, w.vec_d, w.max_eq, w.cg_done,
+                                                                        c.live_count, c.chunk0)));
+    APIC_LAUNCH(CAT_DF_COLS_MUL,
+                (df_cols_mul<N, false><<<g_c, TH, SM, s>>>(t, w.T, w.PF, L.q_row0, L.q_nrow, L.u_row0, L.u_nrow,
+                                                           w.cg_done, 1, c.live_count, c.chunk0)));
+    APIC_LAUNCH(CAT_DF_ROWS_U_GATHER,
+                (df_rows_u_gather<N><<<g_u, TH, SM, s>>>(t, L, w.T, w.vec_w, w.vec_p, w.max_unknown, w.dot_part,
+                                                         w.dot_parts, w.cg_done, 1, c.live_count, c.chunk0)));
+    APIC_LAUNCH(CAT_DF_CG_VECTOR,
+                (df_cg_update<<<B, 256, 0, s>>>(L.n_unknown, w.max_unknown, w.vec_x, w.vec_s, w.vec_p, w.vec_w,
+                                                w.dot_part, w.dot_parts, n_parts, w.cg_scal, w.cg_done, w.cg_iters,
+                                                n_dark_used, led_pos, tol2, c.live_count, c.chunk0)));
   }
-  df_extend<<<dim3((L.n_unknown + 255) / 256, B), 256, 0, s>>>(t, L, w.vec_x, w.max_unknown, w.coef, w.O,
-                                                              c.live_count, c.chunk0);
-  *c.launches += 1;
+  APIC_LAUNCH(CAT_DF_EXTEND, (df_extend<<<dim3((L.n_unknown + 255) / 256, B), 256, 0, s>>>(
+                                 t, L, w.vec_x, w.max_unknown, w.coef, w.O, c.live_count, c.chunk0)));
+#undef APIC_LAUNCH
 }
 
 void launch_darkfield_led(const DevTables& t, const DarkDev& L, int led_pos, int n_dark_used, const Workspace& w,

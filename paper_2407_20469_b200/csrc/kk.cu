@@ -43,11 +43,10 @@ __global__ void __launch_bounds__(256) image_stats_kernel(const float* __restric
   if (threadIdx.x < 3) stats[(size_t(tile) * n_img + img) * 3 + threadIdx.x] = sh[threadIdx.x][0];
 }
 
-void launch_image_stats(const DevTables& t, const float* d_int, int batch, double* stats, cudaStream_t s,
-                        int* launches) {
+void launch_image_stats(const DevTables& t, const float* d_int, int batch, double* stats, const LaunchCtx& c) {
   dim3 grid(t.n_img, batch);
-  image_stats_kernel<<<grid, 256, 0, s>>>(d_int, t.n * t.n, t.n_img, stats);
-  ++*launches;
+  ProfScope ps(c, CAT_STATS);
+  image_stats_kernel<<<grid, 256, 0, c.stream>>>(d_int, t.n * t.n, t.n_img, stats);
 }
 
 // one warp: per-tile status (O1, BASELINE.json item 5, R18) and the ordered list of
@@ -81,10 +80,10 @@ __global__ void tile_status_kernel(const double* __restrict__ stats, int batch, 
 }
 
 void launch_tile_status(const DevTables& t, const double* stats, int batch, int bg_mode, float bg_thr,
-                        int32_t* status, int32_t* live, int32_t* live_count, cudaStream_t s, int* launches) {
-  tile_status_kernel<<<1, 32, 0, s>>>(stats, batch, t.n_img, t.nb, t.n * t.n, bg_mode, bg_thr, status, live,
-                                      live_count);
-  ++*launches;
+                        int32_t* status, int32_t* live, int32_t* live_count, const LaunchCtx& c) {
+  ProfScope ps(c, CAT_STATS);
+  tile_status_kernel<<<1, 32, 0, c.stream>>>(stats, batch, t.n_img, t.nb, t.n * t.n, bg_mode, bg_thr, status, live,
+                                             live_count);
 }
 
 // background / bad-input tiles: outputs are zero
@@ -103,12 +102,13 @@ __global__ void __launch_bounds__(256) zero_dead_kernel(const int32_t* __restric
 }
 
 void launch_zero_dead(const DevTables& t, const int32_t* status, int batch, float* field, float* zern,
-                      float* pupil, cudaStream_t s, int* launches) {
+                      float* pupil, const LaunchCtx& c) {
   const size_t on = size_t(t.n) * t.u;
   dim3 grid(32, batch);
-  zero_dead_kernel<<<grid, 256, 0, s>>>(status, on * on * 2 / 4, t.nz, size_t(t.n) * t.n * 2 / 4,
-                                        reinterpret_cast<float4*>(field), zern, reinterpret_cast<float4*>(pupil));
-  ++*launches;
+  ProfScope ps(c, CAT_STATS);
+  zero_dead_kernel<<<grid, 256, 0, c.stream>>>(status, on * on * 2 / 4, t.nz, size_t(t.n) * t.n * 2 / 4,
+                                               reinterpret_cast<float4*>(field), zern,
+                                               reinterpret_cast<float4*>(pupil));
 }
 
 // ---------------------------------------------------------------------------------- S1-S2
@@ -243,12 +243,15 @@ static void launch_kk_n(const DevTables& t, const Workspace& w, const LaunchCtx&
     attr = true;
   }
   dim3 grid(N / kLines, t.nb, c.chunk_tiles);
-  kk_log_rowfft<N><<<grid, TH, SM, c.stream>>>(t, d_int, stats, floor_rel, w.G, c.live, c.live_count, c.chunk0);
-  kk_col_mask<N><<<grid, TH, SM, c.stream>>>(t, w.G, c.live_count, c.chunk0);
-  kk_row_exp<N><<<grid, TH, SM, c.stream>>>(t, w.G, c.live_count, c.chunk0);
+  { ProfScope ps(c, CAT_KK_LOG_ROWFFT);
+    kk_log_rowfft<N><<<grid, TH, SM, c.stream>>>(t, d_int, stats, floor_rel, w.G, c.live, c.live_count, c.chunk0); }
+  { ProfScope ps(c, CAT_KK_COL_MASK);
+    kk_col_mask<N><<<grid, TH, SM, c.stream>>>(t, w.G, c.live_count, c.chunk0); }
+  { ProfScope ps(c, CAT_KK_ROW_EXP);
+    kk_row_exp<N><<<grid, TH, SM, c.stream>>>(t, w.G, c.live_count, c.chunk0); }
   dim3 grid4((t.bf_max_ncol + kLines - 1) / kLines, t.nb, c.chunk_tiles);
-  kk_col_gather<N><<<grid4, TH, SM, c.stream>>>(t, w.G, w.S, c.live_count, c.chunk0);
-  *c.launches += 4;
+  { ProfScope ps(c, CAT_KK_COL_GATHER);
+    kk_col_gather<N><<<grid4, TH, SM, c.stream>>>(t, w.G, w.S, c.live_count, c.chunk0); }
 }
 
 void launch_kk(const DevTables& t, const Workspace& w, const LaunchCtx& c, const float* d_int, const double* stats,

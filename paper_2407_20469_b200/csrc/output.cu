@@ -95,11 +95,12 @@ static void output_n(const DevTables& t, const Workspace& w, const LaunchCtx& c,
     attr = true;
   }
   dim3 g1((t.known_nrow + kLines - 1) / kLines, t.u, c.chunk_tiles);
-  out_rows<N><<<g1, TH, SM, c.stream>>>(t, w.O, w.TOUT, c.live_count, c.chunk0);
+  { ProfScope ps(c, CAT_OUT_ROWS);
+    out_rows<N><<<g1, TH, SM, c.stream>>>(t, w.O, w.TOUT, c.live_count, c.chunk0); }
   dim3 g2(N * t.u / kLines, t.u, c.chunk_tiles);
-  out_cols<N><<<g2, TH, SM, c.stream>>>(t, w.TOUT, reinterpret_cast<float2*>(d_field), c.live, c.live_count,
-                                        c.chunk0);
-  *c.launches += 2;
+  { ProfScope ps(c, CAT_OUT_COLS);
+    out_cols<N><<<g2, TH, SM, c.stream>>>(t, w.TOUT, reinterpret_cast<float2*>(d_field), c.live, c.live_count,
+                                          c.chunk0); }
 }
 
 void launch_output(const DevTables& t, const Workspace& w, const LaunchCtx& c, float* d_field, float* d_pupil) {
@@ -110,9 +111,9 @@ void launch_output(const DevTables& t, const Workspace& w, const LaunchCtx& c, f
     case 512: output_n<512>(t, w, c, d_field); break;
   }
   if (d_pupil) {
+    ProfScope ps(c, CAT_PUPIL);
     pupil_kernel<<<dim3((t.n_pupil + 255) / 256, c.chunk_tiles), 256, 0, c.stream>>>(
         t, w.coef, reinterpret_cast<float2*>(d_pupil), c.live, c.live_count, c.chunk0);
-    *c.launches += 1;
   }
 }
 

@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdint>
+#include <vector>
 
 #include "geometry.hpp"
 
@@ -87,10 +88,28 @@ struct BatchState {
   int32_t* live_count;     // device scalar
 };
 
+// ------------------------------------------------------------------ per-kernel timing (apic_profile_*)
+enum KernelCat {
+  CAT_STATS = 0, CAT_KK_LOG_ROWFFT, CAT_KK_COL_MASK, CAT_KK_ROW_EXP, CAT_KK_COL_GATHER, CAT_AB_PRODUCTS, CAT_AB_GRAM,
+  CAT_AB_SOLVE, CAT_STITCH, CAT_DF_BUILD_P_ROWS, CAT_DF_COLS_P, CAT_DF_ROWS_RHS, CAT_DF_ROWS_Q, CAT_DF_COLS_MUL,
+  CAT_DF_ROWS_U_SCATTER, CAT_DF_ROWS_U_GATHER, CAT_DF_CG_VECTOR, CAT_DF_EXTEND, CAT_OUT_ROWS, CAT_OUT_COLS,
+  CAT_PUPIL, CAT_COUNT
+};
+
+struct Profiler {
+  bool on = false;
+  int stride = 1;
+  std::vector<cudaEvent_t> ev;     // pool of (start, end) pairs
+  std::vector<int> cat;            // category of each used pair
+  int used = 0;
+  long long launches[CAT_COUNT] = {0};
+};
+
 // ------------------------------------------------------------------ launchers (one per kernel)
 struct LaunchCtx {
   cudaStream_t stream;
   int* launches;           // counter
+  Profiler* prof;
   const int32_t* live;     // compacted tile list
   const int32_t* live_count;
   int chunk0;              // first live-list position of this chunk
@@ -98,11 +117,30 @@ struct LaunchCtx {
 };
 
 // stats / status (batch-level)
-void launch_image_stats(const DevTables& t, const float* d_int, int batch, double* stats, cudaStream_t s, int* launches);
+// Brackets one kernel launch: counts it and, when profiling samples it, records CUDA events around it.
+struct ProfScope {
+  Profiler* p;
+  cudaStream_t s;
+  int slot = -1;
+  ProfScope(const LaunchCtx& c, int cat) : p(c.prof), s(c.stream) {
+    ++*c.launches;
+    if (!p) return;
+    const long long k = p->launches[cat]++;
+    if (!p->on || k % p->stride != 0 || size_t(2 * p->used + 2) > p->ev.size()) return;
+    slot = p->used++;
+    p->cat[slot] = cat;
+    cudaEventRecord(p->ev[2 * slot], s);
+  }
+  ~ProfScope() {
+    if (slot >= 0) cudaEventRecord(p->ev[2 * slot + 1], s);
+  }
+};
+
+void launch_image_stats(const DevTables& t, const float* d_int, int batch, double* stats, const LaunchCtx& c);
 void launch_tile_status(const DevTables& t, const double* stats, int batch, int bg_mode, float bg_thr,
-                        int32_t* status, int32_t* live, int32_t* live_count, cudaStream_t s, int* launches);
+                        int32_t* status, int32_t* live, int32_t* live_count, const LaunchCtx& c);
 void launch_zero_dead(const DevTables& t, const int32_t* status, int batch, float* field, float* zern,
-                      float* pupil, cudaStream_t s, int* launches);
+                      float* pupil, const LaunchCtx& c);
 
 // KK (S1-S5)
 void launch_kk(const DevTables& t, const Workspace& w, const LaunchCtx& c, const float* d_int,
