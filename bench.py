@@ -34,7 +34,6 @@ sys.path.insert(0, ROOT)
 METRIC = "reconstructed output megapixels/sec"
 UNIT = "Mpx/s"
 FP32_LANES_PER_SM = 128          # FMA lanes per SM (4 SMSPs x 32), B200
-DOMINANT = "df_cols_mul"
 
 
 def parse_args():
@@ -46,6 +45,8 @@ def parse_args():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (2 = default workload)")
     ap.add_argument("--tiles", type=int, default=0, help="tiles per step and per GPU (0 = the config's batch, capped at 64)")
     ap.add_argument("--chunk", type=int, default=0, help="apic_params.chunk_tiles (0 = library default)")
+    ap.add_argument("--df-mode", type=int, default=0, help="darkfield scheduler: 0 persistent task kernel, 1 launch per phase")
+    ap.add_argument("--df-tol", type=float, default=-1.0, help="CG tolerance (default: the library's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--breakdown", action="store_true", help="also print the per-kernel time table to stderr")
@@ -197,7 +198,8 @@ def main():
     reps = -(-tiles // n_gen)
     host = np.concatenate([stacks] * reps)[:tiles]
     x = torch.from_numpy(host).cuda()
-    plan = A.Plan.from_config(cfg, max_batch=tiles, chunk_tiles=args.chunk)
+    popts = {"df_tol": args.df_tol} if args.df_tol > 0 else {}
+    plan = A.Plan.from_config(cfg, max_batch=tiles, chunk_tiles=args.chunk, df_mode=args.df_mode, **popts)
     n, on, nz = cfg.tile_n, cfg.out_n, plan.nz
     out = (torch.empty((tiles, on, on), dtype=torch.complex64, device="cuda"),
            torch.empty((tiles, nz), dtype=torch.float32, device="cuda"),
@@ -218,7 +220,7 @@ def main():
         vis = os.environ["CUDA_VISIBLE_DEVICES"].split(",")
         sampler.gpu_id = vis[local] if local < len(vis) else str(local)
     sampler.start()
-    plan.profile_begin(stride=4, max_samples=16384)
+    plan.profile_begin(stride=1 if args.df_mode == 0 else 4, max_samples=16384)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches = 0
     barrier()
@@ -239,27 +241,36 @@ def main():
     live = int((status != 1).sum())
     mpx = world * args.steps * tiles * on * on / 1e6 / (ms / 1e3)
 
-    # ---- roofline of the dominant kernel: executed flops per launch / event time
+    # ---- roofline of the dominant kernel: executed flops / CUDA-event time
     chunk = plan.info["chunk_tiles"]
-    ms_sum, samples, nlaunch = prof[DOMINANT]
     fft_line = 5.0 * n * math.log2(n)                    # flop of one N-point complex FFT (5 N log2 N)
-    flop_per_tile_launch = 2 * n * fft_line + 6.0 * n * n  # N columns x (IFFT + FFT) + complex multiply
-    tiles_per_launch = min(chunk, tiles)                 # all but the ragged last chunk
-    n_chunks = -(-tiles // chunk)
-    avg_tiles = tiles / n_chunks
-    avg_ms = ms_sum / max(samples, 1)
-    achieved = flop_per_tile_launch * avg_tiles / (avg_ms * 1e-3) / 1e12 if samples else None
     sm_max = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
     sms = torch.cuda.get_device_properties(local).multi_processor_count
     peak = sms * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     total_kernel_ms = sum(v[0] / max(v[1], 1) * v[2] for v in prof.values())
+    dominant = "df_persistent" if args.df_mode == 0 and cfg.n_dark else "df_cols_mul"
+    if not cfg.n_dark:
+        dominant = max(prof, key=lambda k: prof[k][0] / max(prof[k][1], 1) * prof[k][2])
+    ms_sum, samples, nlaunch = prof[dominant]
+    avg_ms = ms_sum / max(samples, 1)
+    if dominant == "df_persistent":
+        # executed work counted by the kernel itself: N-point line transforms of all its strip tasks
+        lines = plan.profile_work()
+        flop_per_launch = lines * fft_line / max(nlaunch, 1)
+        note = f"{lines} executed {n}-point line FFTs x 5 N log2 N over {nlaunch} launches (pointwise work not counted)"
+    elif dominant == "df_cols_mul":
+        n_chunks = -(-tiles // chunk)
+        flop_per_launch = (2 * n * fft_line + 6.0 * n * n) * tiles / n_chunks
+        note = "N columns x (IFFT + FFT) x 5 N log2 N + complex multiply, per tile of the launch"
+    else:
+        flop_per_launch, note = None, "no flop model for this kernel"
+    achieved = flop_per_launch / (avg_ms * 1e-3) / 1e12 if (samples and flop_per_launch) else None
     share = (avg_ms * nlaunch / total_kernel_ms) if total_kernel_ms else None
-    roofline = {"kernel": DOMINANT, "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+    roofline = {"kernel": dominant, "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                 "frac": (achieved / peak) if achieved else None, "traffic": None,
                 "avg_launch_ms": avg_ms, "sampled_launches": int(samples), "launches": int(nlaunch),
-                "share_of_kernel_time": share,
+                "share_of_kernel_time": share, "flop_per_launch": flop_per_launch, "flop_model": note,
                 "peak_note": f"{sms} SMs x {FP32_LANES_PER_SM} FMA lanes x 2 x {sm_max:.0f} MHz (derived, DESIGN.md §5)",
-                "flop_per_launch": flop_per_tile_launch * avg_tiles,
                 "hbm_peak_gbs_measured": peaks.get("hbm_gbs")}
     if args.breakdown and rank == 0:
         print(f"{'kernel':22s} {'launches':>9s} {'avg us':>9s} {'est ms/step':>12s} {'share':>7s}", file=sys.stderr)

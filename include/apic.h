@@ -74,6 +74,9 @@ typedef struct {
                             min(max_batch, internal chunk)                                       */
   int chunk_tiles;       /* tiles per internal pass; 0 = chosen so that one pass's transform
                             working set stays inside the 126 MB L2                              */
+  int df_mode;           /* darkfield scheduler: 0 = persistent task kernel (one launch per LED and
+                            pass, stops when every tile has converged), 1 = one launch per phase
+                            (df_iters iterations are always enqueued)                            */
 } apic_params;
 
 /* Fills *p with the defaults (kk_pad 1, refine_iters 3, df_iters 48, df_tol 1e-5, floor 1e-6,
@@ -167,6 +170,9 @@ int apic_profile_categories(void);
 const char* apic_profile_category_name(int cat);
 int apic_profile_begin(apic_plan* plan, int stride, int max_samples);
 int apic_profile_end(apic_plan* plan, double* ms_sum, long long* samples, long long* launches);
+/* Number of N-point line transforms executed by the persistent darkfield kernels since
+ * apic_profile_begin (synchronises the device). */
+int apic_profile_work(apic_plan* plan, unsigned long long* line_transforms);
 
 const char* apic_strerror(int err);
 const char* apic_last_cuda_error(void);

@@ -24,7 +24,7 @@ EXPORTS = ("apic_params_default", "apic_plan_create", "apic_plan_destroy", "apic
            "apic_geometry_info", "apic_plan_dark_sets", "apic_reconstruct", "apic_reconstruct_host",
            "apic_debug_buffer", "apic_debug_copy", "apic_fft2d", "apic_last_launch_count", "apic_strerror",
            "apic_last_cuda_error", "apic_version", "apic_profile_categories", "apic_profile_category_name",
-           "apic_profile_begin", "apic_profile_end")
+           "apic_profile_begin", "apic_profile_end", "apic_profile_work")
 
 
 class ApicError(RuntimeError):
@@ -38,7 +38,7 @@ class ApicParams(C.Structure):
                 ("n_zernike", C.c_int), ("noll", C.POINTER(C.c_int)), ("kk_pad", C.c_int),
                 ("refine_iters", C.c_int), ("df_iters", C.c_int), ("df_tol", C.c_float),
                 ("intensity_floor", C.c_float), ("bg_mode", C.c_int), ("bg_threshold", C.c_float),
-                ("max_batch", C.c_int), ("chunk_tiles", C.c_int)]
+                ("max_batch", C.c_int), ("chunk_tiles", C.c_int), ("df_mode", C.c_int)]
 
 
 class PlanInfo(C.Structure):
@@ -87,6 +87,7 @@ def load() -> C.CDLL:
     lib.apic_profile_begin.argtypes = [C.c_void_p, C.c_int, C.c_int]
     lib.apic_profile_end.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_longlong),
                                      C.POINTER(C.c_longlong)]
+    lib.apic_profile_work.argtypes = [C.c_void_p, C.POINTER(C.c_ulonglong)]
     _lib = lib
     return lib
 
@@ -232,6 +233,12 @@ class Plan:
         ms, sm, la = (C.c_double * n)(), (C.c_longlong * n)(), (C.c_longlong * n)()
         _check(self._lib.apic_profile_end(self._h, ms, sm, la), "apic_profile_end")
         return {self._lib.apic_profile_category_name(i).decode(): (ms[i], sm[i], la[i]) for i in range(n)}
+
+    def profile_work(self) -> int:
+        """N-point line transforms executed by the persistent darkfield kernels since profile_begin."""
+        v = C.c_ulonglong()
+        _check(self._lib.apic_profile_work(self._h, C.byref(v)), "apic_profile_work")
+        return int(v.value)
 
     @property
     def last_launch_count(self) -> int:

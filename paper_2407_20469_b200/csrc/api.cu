@@ -95,6 +95,7 @@ void apic_params_default(apic_params* p) {
   p->bg_threshold = 0.f;
   p->max_batch = 64;
   p->chunk_tiles = 0;
+  p->df_mode = 0;
 }
 
 const char* apic_strerror(int err) {
@@ -251,6 +252,9 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
   ok = ok && plan->dalloc(&w.cg_scal, c * 4, false);
   ok = ok && plan->dalloc(&w.cg_done, c, false);
   ok = ok && plan->dalloc(&w.cg_iters, c * std::max<size_t>(1, h.dark.size()), false);
+  ok = ok && plan->dalloc(&w.df_sync, c + 2, false);
+  ok = ok && plan->dalloc(&w.df_work, 1, false);
+  if (ok) ok = cuda_ok(cudaMemset(w.df_work, 0, sizeof(unsigned long long)), "cudaMemset");
   ok = ok && plan->dalloc(&w.TOUT, c * nn * h.u, false);
   ok = ok && plan->dalloc(&plan->bs.stats, size_t(p->max_batch) * d.n_img * 3, false);
   ok = ok && plan->dalloc(&plan->bs.live, size_t(p->max_batch), false);
@@ -318,7 +322,8 @@ int apic_reconstruct(apic_plan* plan, const float* d_intensity, int batch, float
     launch_aberration(t, w, c, p.refine_iters, d_zernike, d_status);                          // S6
     launch_stitch(t, w, c);                                                                   // S7
     for (int k = 0; k < n_dark_used; ++k)                                                     // S8-S10
-      launch_darkfield_led(t, plan->dark[k], k, std::max(1, n_dark_used), w, c, d_intensity, p.df_iters, p.df_tol);
+      launch_darkfield_led(t, plan->dark[k], k, std::max(1, n_dark_used), w, c, d_intensity, p.df_iters, p.df_tol,
+                           p.df_mode);
     launch_output(t, w, c, d_field, d_pupil);                                                 // S10
   }
   if (!cuda_ok(cudaGetLastError(), "apic_reconstruct launch")) return APIC_ECUDA;
@@ -410,7 +415,8 @@ int apic_last_launch_count(const apic_plan* plan) { return plan ? plan->launches
 static const char* kCatNames[CAT_COUNT] = {
     "stats_status", "kk_log_rowfft", "kk_col_mask", "kk_row_exp", "kk_col_gather", "ab_pair_products", "ab_gram",
     "ab_solve", "stitch", "df_build_p_rows", "df_cols_p", "df_rows_rhs", "df_rows_q", "df_cols_mul",
-    "df_rows_u_scatter", "df_rows_u_gather", "df_cg_vector", "df_extend", "out_rows", "out_cols", "pupil"};
+    "df_rows_u_scatter", "df_rows_u_gather", "df_cg_vector", "df_extend", "out_rows", "out_cols", "pupil",
+    "df_persistent"};
 
 int apic_profile_categories(void) { return CAT_COUNT; }
 const char* apic_profile_category_name(int cat) { return (cat >= 0 && cat < CAT_COUNT) ? kCatNames[cat] : ""; }
@@ -428,6 +434,15 @@ int apic_profile_begin(apic_plan* plan, int stride, int max_samples) {
   pr.stride = stride;
   for (long long& v : pr.launches) v = 0;
   pr.on = true;
+  if (!cuda_ok(cudaMemset(plan->ws.df_work, 0, sizeof(unsigned long long)), "cudaMemset")) return APIC_ECUDA;
+  return APIC_OK;
+}
+
+int apic_profile_work(apic_plan* plan, unsigned long long* line_transforms) {
+  if (!plan || !line_transforms) return APIC_EINVAL;
+  if (!cuda_ok(cudaMemcpy(line_transforms, plan->ws.df_work, sizeof(unsigned long long), cudaMemcpyDeviceToHost),
+               "apic_profile_work"))
+    return APIC_ECUDA;
   return APIC_OK;
 }
 

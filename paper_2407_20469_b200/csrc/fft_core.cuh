@@ -120,10 +120,11 @@ struct RegDft<16, INV> {
 
 // ---- per-N factorisation
 template <int N> struct FftCfg;
-template <> struct FftCfg<64>  { static constexpr int R1 = 8,  R2 = 8,  R3 = 1, THREADS = 128; };
-template <> struct FftCfg<128> { static constexpr int R1 = 16, R2 = 8,  R3 = 1, THREADS = 128; };
-template <> struct FftCfg<256> { static constexpr int R1 = 16, R2 = 16, R3 = 1, THREADS = 256; };
-template <> struct FftCfg<512> { static constexpr int R1 = 8,  R2 = 8,  R3 = 8, THREADS = 512; };
+// MINB = CTAs per SM the strip kernels are compiled for (register cap = 64K / (THREADS * MINB))
+template <> struct FftCfg<64>  { static constexpr int R1 = 8,  R2 = 8,  R3 = 1, THREADS = 128, MINB = 8; };
+template <> struct FftCfg<128> { static constexpr int R1 = 16, R2 = 8,  R3 = 1, THREADS = 128, MINB = 8; };
+template <> struct FftCfg<256> { static constexpr int R1 = 16, R2 = 16, R3 = 1, THREADS = 256, MINB = 4; };
+template <> struct FftCfg<512> { static constexpr int R1 = 8,  R2 = 8,  R3 = 8, THREADS = 512, MINB = 1; };
 
 // One Stockham pass over all kLines lines of the strip, in place (read all -> sync -> write all).
 template <int N, int R, int NS, bool INV>

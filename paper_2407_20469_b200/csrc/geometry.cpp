@@ -123,6 +123,7 @@ bool build_geometry(const apic_params& p, HostTables& t, std::string& err) {
   if (p.df_iters < 1) { err = "df_iters must be >= 1"; return false; }
   if (p.bg_mode < 0 || p.bg_mode > 2) { err = "bg_mode must be 0, 1 or 2"; return false; }
   if (p.max_batch < 1) { err = "max_batch must be >= 1"; return false; }
+  if (p.df_mode < 0 || p.df_mode > 1) { err = "df_mode must be 0 (persistent) or 1 (multi-launch)"; return false; }
   for (int a = 0; a < p.n_zernike; ++a) {
     if (p.noll[a] < 4) { err = "Noll indices must be >= 4 (piston/tilt are the null space of Eq. 10)"; return false; }
     for (int b = 0; b < a; ++b)

@@ -77,6 +77,8 @@ struct Workspace {
   float* cg_scal;          // [chunk][4]: gamma, gamma0, -, -
   int32_t* cg_done;        // [chunk]
   int32_t* cg_iters;       // [chunk][n_dark_used]
+  int32_t* df_sync;        // [2 + chunk] persistent scheduler: ticket, finished tiles, per-tile progress
+  unsigned long long* df_work;   // [1] line transforms executed by the persistent darkfield kernels
   float2* TOUT;            // [chunk][N][uN]
   int max_eq, max_unknown;
 };
@@ -93,7 +95,7 @@ enum KernelCat {
   CAT_STATS = 0, CAT_KK_LOG_ROWFFT, CAT_KK_COL_MASK, CAT_KK_ROW_EXP, CAT_KK_COL_GATHER, CAT_AB_PRODUCTS, CAT_AB_GRAM,
   CAT_AB_SOLVE, CAT_STITCH, CAT_DF_BUILD_P_ROWS, CAT_DF_COLS_P, CAT_DF_ROWS_RHS, CAT_DF_ROWS_Q, CAT_DF_COLS_MUL,
   CAT_DF_ROWS_U_SCATTER, CAT_DF_ROWS_U_GATHER, CAT_DF_CG_VECTOR, CAT_DF_EXTEND, CAT_OUT_ROWS, CAT_OUT_COLS,
-  CAT_PUPIL, CAT_COUNT
+  CAT_PUPIL, CAT_DF_PERSISTENT, CAT_COUNT
 };
 
 struct Profiler {
@@ -151,7 +153,7 @@ void launch_aberration(const DevTables& t, const Workspace& w, const LaunchCtx& 
 void launch_stitch(const DevTables& t, const Workspace& w, const LaunchCtx& c);
 // darkfield (S8-S10) for one LED
 void launch_darkfield_led(const DevTables& t, const DarkDev& L, int led_pos, int n_dark_used, const Workspace& w,
-                          const LaunchCtx& c, const float* d_int, int df_iters, float df_tol);
+                          const LaunchCtx& c, const float* d_int, int df_iters, float df_tol, int df_mode);
 // outputs
 void launch_output(const DevTables& t, const Workspace& w, const LaunchCtx& c, float* d_field, float* d_pupil);
 

@@ -87,13 +87,15 @@ def test_single_tile_configs(A, index):
 
 
 # ---------------------------------------------------------------------------------- config 2
-def test_config2_reduced_all_tiles_ragged_chunks(A):
+@pytest.mark.parametrize("df_mode", [0, 1])
+def test_config2_reduced_all_tiles_ragged_chunks(A, df_mode):
     """64x64 variant of config 2 (8 + 16 LEDs, Poisson noise, 3x grid): every tile against the
-    oracle, with 5 tiles over chunks of 2 (two full chunks and a ragged tail)."""
+    oracle, with 5 tiles over chunks of 2 (two full chunks and a ragged tail); both darkfield
+    schedulers (persistent task kernel / one launch per phase)."""
     cfg = get_config(2, tile_n=64, batch=5, grid=(3, 2))
     stacks, _ = make_batch(cfg, range(5))
     refs, _ = oracle_reconstruct(cfg, stacks)
-    plan, field, zern, pupil, status = gpu_reconstruct(A, cfg, stacks, chunk_tiles=2)
+    plan, field, zern, pupil, status = gpu_reconstruct(A, cfg, stacks, chunk_tiles=2, df_mode=df_mode)
     assert plan.info["chunk_tiles"] == 2
     for b in range(5):
         check_tile(refs[b], field[b], zern[b], pupil[b], status[b], f"cfg2@64 tile {b}")
@@ -101,11 +103,12 @@ def test_config2_reduced_all_tiles_ragged_chunks(A):
     assert its.min() >= 1 and its.max() < 48          # CG converged by its tolerance, not the cap
 
 
-def test_config2_128(A):
+@pytest.mark.parametrize("df_mode", [0, 1])
+def test_config2_128(A, df_mode):
     cfg = get_config(2, tile_n=128, batch=3, grid=(2, 2))
     stacks, _ = make_batch(cfg, range(3))
     refs, _ = oracle_reconstruct(cfg, stacks)
-    _, field, zern, pupil, status = gpu_reconstruct(A, cfg, stacks)
+    _, field, zern, pupil, status = gpu_reconstruct(A, cfg, stacks, df_mode=df_mode)
     for b in range(3):
         check_tile(refs[b], field[b], zern[b], pupil[b], status[b], f"cfg2@128 tile {b}")
 
@@ -210,6 +213,8 @@ def test_results_are_bit_reproducible_and_batch_invariant(A):
     assert np.array_equal(f1, f2) and np.array_equal(z1, z2)
     _, f3, z3, _, _ = gpu_reconstruct(A, cfg, stacks[::-1].copy(), chunk_tiles=3)
     assert np.array_equal(f1, f3[::-1]) and np.array_equal(z1, z3[::-1])
+    _, f4, z4, _, _ = gpu_reconstruct(A, cfg, stacks, df_mode=1)      # the other scheduler: same arithmetic
+    assert np.array_equal(f1, f4) and np.array_equal(z1, z4)
 
 
 def test_host_entry_point_and_batch_limits(A):
