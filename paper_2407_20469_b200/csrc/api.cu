@@ -163,11 +163,8 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
   bool ok = true;
   // twiddles and output ramps, fp64 -> fp32
   {
-    std::vector<float2> tw(n);
-    for (int m = 0; m < n; ++m) {
-      const double a = -2.0 * M_PI * m / n;
-      tw[m] = make_float2(float(std::cos(a)), float(std::sin(a)));
-    }
+    std::vector<float2> tw;
+    build_twiddles(n, tw);
     ok = ok && plan->upload(&d.tw, tw);
     std::vector<float2> ramp(size_t(h.u) * n);
     for (int a = 0; a < h.u; ++a)
@@ -215,7 +212,7 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
     plan->dark.push_back(q);
     max_eq = std::max(max_eq, L.n_eq);
     max_unknown = std::max(max_unknown, L.n_unknown);
-    dot_parts = std::max(dot_parts, (L.u_nrow + kLines - 1) / kLines);
+    dot_parts = std::max(dot_parts, (L.u_nrow + strip_lines(n) - 1) / strip_lines(n));
   }
   // ---- workspace
   Workspace& w = plan->ws;
@@ -224,7 +221,7 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
   if (chunk <= 0) {
     // darkfield CG working set per tile: T rows in use (<= 2/3 N) + p (N^2)  ~ 1.7 N^2 complex64
     const double per_tile = 1.7 * double(nn) * sizeof(float2);
-    chunk = int(56.0e6 / per_tile);
+    chunk = int(64.0e6 / per_tile);
     chunk = std::max(8, std::min(chunk, 512));
   }
   chunk = std::max(1, std::min(chunk, p->max_batch));
@@ -315,9 +312,12 @@ int apic_reconstruct(apic_plan* plan, const float* d_intensity, int batch, float
     n_live = *plan->h_live_count;
   }
   const int n_dark_used = int(plan->dark.size());
-  for (int c0 = 0; c0 < n_live; c0 += w.chunk) {
+  // balanced passes: ceil(n_live / chunk) passes of (almost) equal size
+  const int n_pass = (n_live + w.chunk - 1) / w.chunk;
+  const int per_pass = n_pass ? (n_live + n_pass - 1) / n_pass : 0;
+  for (int c0 = 0; c0 < n_live; c0 += per_pass) {
     LaunchCtx c{s, &plan->launches, &plan->prof, plan->bs.live, plan->bs.live_count, c0,
-                std::min(w.chunk, n_live - c0)};
+                std::min(per_pass, n_live - c0)};
     launch_kk(t, w, c, d_intensity, plan->bs.stats, p.intensity_floor);                       // S1-S5
     launch_aberration(t, w, c, p.refine_iters, d_zernike, d_status);                          // S6
     launch_stitch(t, w, c);                                                                   // S7
@@ -397,13 +397,10 @@ int apic_fft2d(float* d_data, int n, int batch, int inverse, void* cuda_stream) 
   static float2* tw_cache[4] = {nullptr, nullptr, nullptr, nullptr};
   const int slot = n == 64 ? 0 : n == 128 ? 1 : n == 256 ? 2 : 3;
   if (!tw_cache[slot]) {
-    std::vector<float2> tw(n);
-    for (int m = 0; m < n; ++m) {
-      const double a = -2.0 * M_PI * m / n;
-      tw[m] = make_float2(float(std::cos(a)), float(std::sin(a)));
-    }
-    if (!cuda_ok(cudaMalloc(reinterpret_cast<void**>(&tw_cache[slot]), n * sizeof(float2)), "cudaMalloc")) return APIC_ECUDA;
-    if (!cuda_ok(cudaMemcpy(tw_cache[slot], tw.data(), n * sizeof(float2), cudaMemcpyHostToDevice), "cudaMemcpy")) return APIC_ECUDA;
+    std::vector<float2> tw;
+    build_twiddles(n, tw);
+    if (!cuda_ok(cudaMalloc(reinterpret_cast<void**>(&tw_cache[slot]), tw.size() * sizeof(float2)), "cudaMalloc")) return APIC_ECUDA;
+    if (!cuda_ok(cudaMemcpy(tw_cache[slot], tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice), "cudaMemcpy")) return APIC_ECUDA;
   }
   launch_fft2d(reinterpret_cast<float2*>(d_data), n, batch, inverse != 0, tw_cache[slot], static_cast<cudaStream_t>(cuda_stream));
   if (!cuda_ok(cudaGetLastError(), "apic_fft2d")) return APIC_ECUDA;

@@ -72,69 +72,80 @@ __device__ __forceinline__ float block_sum(float v, float* red) {
   return s;
 }
 
+// centred-row window test on an FFT-order row index
+template <int N>
+__device__ __forceinline__ bool in_rows(int fy, int row0, int nrow) {
+  const int ky = fy < N / 2 ? fy : fy - N;
+  return unsigned(ky - row0) < unsigned(nrow);
+}
+template <int N>
+__device__ __forceinline__ int col_of(int fx, int col0) { return (fx < N / 2 ? fx : fx - N) - col0; }
+
 // ---------------------------------------------------------------- P0: P_hat rows -> row IFFT
 template <int N>
 __device__ __forceinline__ void task_build_p_rows(const DfArgs& a, int slot, int strip, float2* sm, float* c_sh) {
-  constexpr int TH = FftCfg<N>::THREADS;
+  using S = Strip<N>;
+  using TH = StripThread<N, false>;
   const DarkDev& L = a.L;
-  const int r0 = strip * kLines, nz = a.t.nz;
+  const int nz = a.t.nz, line = TH::line(), tt = TH::t(), row = strip * S::LINES + line;
+  __syncthreads();
   if (threadIdx.x < nz) c_sh[threadIdx.x] = a.coef[size_t(slot) * nz + threadIdx.x];
-  strip_zero<N>(sm);
   __syncthreads();
-  const float2* o = a.O_in + size_t(slot) * (N * N);
-  for (int idx = threadIdx.x; idx < kLines * L.d_ncol; idx += TH) {
-    const int l = idx / L.d_ncol, c = idx % L.d_ncol;
-    if (r0 + l >= L.d_nrow) continue;
-    const int fy = wrapN(L.d_row0 + r0 + l, N);
-    const int e = L.dmap[fy * L.d_ncol + c];
-    if (e < L.n_unknown) continue;                                     // not in P (unknown or outside)
-    const int fx = wrapN(L.d_col0 + c, N);
-    const float phi = zern_phase(L.zern + size_t(e) * nz, c_sh, nz);
-    float sn, cs;
-    sincosf(phi, &sn, &cs);
-    strip_at<N>(sm, l, fx) = cmul(o[fy * N + fx], make_float2(cs, sn));
+  const bool valid = row < L.d_nrow;
+  const int fy = wrapN(L.d_row0 + row, N);
+  const float2* o = a.O_in + size_t(slot) * (N * N) + fy * N;
+  float2 v[S::R];
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) {
+    const int fx = tt + S::TPL * r, c = col_of<N>(fx, L.d_col0);
+    v[r] = make_float2(0.f, 0.f);
+    if (valid && unsigned(c) < unsigned(L.d_ncol)) {
+      const int e = __ldg(&L.dmap[fy * L.d_ncol + c]);
+      if (e >= L.n_unknown) {                                          // in P = D_i ∩ known
+        const float phi = zern_phase(L.zern + size_t(e) * nz, c_sh, nz);
+        float sn, cs;
+        sincosf(phi, &sn, &cs);
+        v[r] = cmul(o[fx], make_float2(cs, sn));
+      }
+    }
   }
-  __syncthreads();
-  fft_lines<N, true>(sm, a.t.tw);
-  float2* tt = a.T + size_t(slot) * (N * N);
-  for (int idx = threadIdx.x; idx < kLines * N; idx += TH) {
-    const int l = idx / N, e = idx % N;
-    if (r0 + l >= L.d_nrow) continue;
-    tt[wrapN(L.d_row0 + r0 + l, N) * N + e] = strip_at<N>(sm, l, e);
+  fft_regs<N, true>(v, sm + line * S::LS, tt, a.t.tw);
+  if (valid) {
+    float2* tr = a.T + size_t(slot) * (N * N) + fy * N;
+#pragma unroll
+    for (int r = 0; r < S::R; ++r) tr[tt + S::TPL * r] = v[r];
   }
 }
 
 // ---------------------------------------------------------------- P1: p, I - |p|^2, column FFT
 template <int N>
 __device__ __forceinline__ void task_cols_p(const DfArgs& a, int slot, int tile, int strip, float2* sm) {
-  constexpr int TH = FftCfg<N>::THREADS;
+  using S = Strip<N>;
+  using TH = StripThread<N, true>;
   const DarkDev& L = a.L;
-  const int x0 = strip * kLines;
-  strip_zero<N>(sm);
-  __syncthreads();
-  float2* tt = a.T + size_t(slot) * (N * N);
-  for (int idx = threadIdx.x; idx < kLines * L.d_nrow; idx += TH) {
-    const int l = idx % kLines, r = idx / kLines;
-    const int fy = wrapN(L.d_row0 + r, N);
-    strip_at<N>(sm, l, fy) = ldcg2(&tt[fy * N + x0 + l]);
+  const int line = TH::line(), tt = TH::t(), x = strip * S::LINES + line;
+  float2* tc = a.T + size_t(slot) * (N * N) + x;
+  float2 v[S::R];
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) {
+    const int fy = tt + S::TPL * r;
+    v[r] = in_rows<N>(fy, L.d_row0, L.d_nrow) ? ldcg2(&tc[fy * N]) : make_float2(0.f, 0.f);
   }
-  __syncthreads();
-  fft_lines<N, true>(sm, a.t.tw);
-  const float* img = a.d_int + (size_t(tile) * a.t.n_img + a.t.nb + L.led) * (N * N);
-  float2* pf = a.PF + size_t(slot) * (N * N);
-  for (int idx = threadIdx.x; idx < kLines * N; idx += TH) {
-    const int l = idx % kLines, e = idx / kLines;
-    float2& v = strip_at<N>(sm, l, e);
-    const float2 p = v;
-    pf[e * N + x0 + l] = p;
-    v = make_float2(__ldg(&img[e * N + x0 + l]) - (p.x * p.x + p.y * p.y), 0.f);   // Eq. 13 lhs, spatial
+  fft_regs<N, true>(v, sm + line * S::LS, tt, a.t.tw);
+  const float* img = a.d_int + (size_t(tile) * a.t.n_img + a.t.nb + L.led) * (N * N) + x;
+  float2* pf = a.PF + size_t(slot) * (N * N) + x;
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) {
+    const int y = tt + S::TPL * r;
+    const float2 p = v[r];
+    pf[y * N] = p;
+    v[r] = make_float2(__ldg(&img[y * N]) - (p.x * p.x + p.y * p.y), 0.f);       // Eq. 13 lhs, spatial
   }
-  __syncthreads();
-  fft_lines<N, false>(sm, a.t.tw);
-  for (int idx = threadIdx.x; idx < kLines * L.q_nrow; idx += TH) {
-    const int l = idx % kLines, r = idx / kLines;
-    const int fy = wrapN(L.q_row0 + r, N);
-    tt[fy * N + x0 + l] = strip_at<N>(sm, l, fy);
+  fft_regs<N, false>(v, sm + line * S::LS, tt, a.t.tw);
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) {
+    const int fy = tt + S::TPL * r;
+    if (in_rows<N>(fy, L.q_row0, L.q_nrow)) tc[fy * N] = v[r];
   }
 }
 
@@ -142,96 +153,89 @@ __device__ __forceinline__ void task_cols_p(const DfArgs& a, int slot, int tile,
 // row FFT, keep the bins of Q only (x 1/N^2), row IFFT.  In P2 this turns F(I-|p|^2) into M_Q d.
 template <int N>
 __device__ __forceinline__ void task_rows_q(const DfArgs& a, int slot, int strip, float2* sm) {
-  constexpr int TH = FftCfg<N>::THREADS;
+  using S = Strip<N>;
+  using TH = StripThread<N, false>;
   const DarkDev& L = a.L;
-  const int r0 = strip * kLines;
-  float2* tt = a.T + size_t(slot) * (N * N);
-  for (int idx = threadIdx.x; idx < kLines * N; idx += TH) {
-    const int l = idx / N, e = idx % N;
-    float2 v = make_float2(0.f, 0.f);
-    if (r0 + l < L.q_nrow) v = ldcg2(&tt[wrapN(L.q_row0 + r0 + l, N) * N + e]);
-    strip_at<N>(sm, l, e) = v;
-  }
-  __syncthreads();
-  fft_lines<N, false>(sm, a.t.tw);
+  const int line = TH::line(), tt = TH::t(), row = strip * S::LINES + line;
+  const bool valid = row < L.q_nrow;
+  const int fy = wrapN(L.q_row0 + row, N);
+  float2* tr = a.T + size_t(slot) * (N * N) + fy * N;
+  float2 v[S::R];
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) v[r] = valid ? ldcg2(&tr[tt + S::TPL * r]) : make_float2(0.f, 0.f);
+  fft_regs<N, false>(v, sm + line * S::LS, tt, a.t.tw);
   const float scale = 1.f / float(N * N);
-  for (int idx = threadIdx.x; idx < kLines * N; idx += TH) {
-    const int l = idx / N, fx = idx % N;
-    float2& v = strip_at<N>(sm, l, fx);
-    bool in = false;
-    if (r0 + l < L.q_nrow) {
-      const int kx = fx < N / 2 ? fx : fx - N;
-      const int c = kx - L.q_col0;
-      if (c >= 0 && c < L.q_ncol) in = __ldg(&L.qmap[wrapN(L.q_row0 + r0 + l, N) * L.q_ncol + c]) >= 0;
-    }
-    v = in ? cscale(v, scale) : make_float2(0.f, 0.f);
+  const int32_t* qrow = L.qmap + fy * L.q_ncol;
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) {
+    const int c = col_of<N>(tt + S::TPL * r, L.q_col0);
+    const bool in = valid && unsigned(c) < unsigned(L.q_ncol) && __ldg(&qrow[c]) >= 0;
+    v[r] = in ? cscale(v[r], scale) : make_float2(0.f, 0.f);
   }
-  __syncthreads();
-  fft_lines<N, true>(sm, a.t.tw);
-  for (int idx = threadIdx.x; idx < kLines * N; idx += TH) {
-    const int l = idx / N, e = idx % N;
-    if (r0 + l >= L.q_nrow) continue;
-    tt[wrapN(L.q_row0 + r0 + l, N) * N + e] = strip_at<N>(sm, l, e);
+  fft_regs<N, true>(v, sm + line * S::LS, tt, a.t.tw);
+  if (valid) {
+#pragma unroll
+    for (int r = 0; r < S::R; ++r) tr[tt + S::TPL * r] = v[r];
   }
 }
 
 // ---------------------------------------------------------------- B / D / P3: column IFFT, . p or conj p, column FFT
 template <int N, bool CONJ>
 __device__ __forceinline__ void task_cols_mul(const DfArgs& a, int slot, int strip, float2* sm) {
-  constexpr int TH = FftCfg<N>::THREADS;
+  using S = Strip<N>;
+  using TH = StripThread<N, true>;
   const DarkDev& L = a.L;
   const int in_row0 = CONJ ? L.u_row0 : L.q_row0, in_nrow = CONJ ? L.u_nrow : L.q_nrow;
   const int out_row0 = CONJ ? L.q_row0 : L.u_row0, out_nrow = CONJ ? L.q_nrow : L.u_nrow;
-  const int x0 = strip * kLines;
-  strip_zero<N>(sm);
-  __syncthreads();
-  float2* tt = a.T + size_t(slot) * (N * N);
-  for (int idx = threadIdx.x; idx < kLines * in_nrow; idx += TH) {
-    const int l = idx % kLines, r = idx / kLines;
-    const int fy = wrapN(in_row0 + r, N);
-    strip_at<N>(sm, l, fy) = ldcg2(&tt[fy * N + x0 + l]);
+  const int line = TH::line(), tt = TH::t(), x = strip * S::LINES + line;
+  float2* tc = a.T + size_t(slot) * (N * N) + x;
+  float2 v[S::R];
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) {
+    const int fy = tt + S::TPL * r;
+    v[r] = in_rows<N>(fy, in_row0, in_nrow) ? ldcg2(&tc[fy * N]) : make_float2(0.f, 0.f);
   }
-  __syncthreads();
-  fft_lines<N, true>(sm, a.t.tw);
-  const float2* pf = a.PF + size_t(slot) * (N * N);
-  for (int idx = threadIdx.x; idx < kLines * N; idx += TH) {
-    const int l = idx % kLines, e = idx / kLines;
-    float2& v = strip_at<N>(sm, l, e);
-    const float2 p = ldcg2(&pf[e * N + x0 + l]);
-    v = CONJ ? cmulc(v, p) : cmul(v, p);
+  fft_regs<N, true>(v, sm + line * S::LS, tt, a.t.tw);
+  const float2* pf = a.PF + size_t(slot) * (N * N) + x;
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) {
+    const float2 p = ldcg2(&pf[(tt + S::TPL * r) * N]);
+    v[r] = CONJ ? cmulc(v[r], p) : cmul(v[r], p);
   }
-  __syncthreads();
-  fft_lines<N, false>(sm, a.t.tw);
-  for (int idx = threadIdx.x; idx < kLines * out_nrow; idx += TH) {
-    const int l = idx % kLines, r = idx / kLines;
-    const int fy = wrapN(out_row0 + r, N);
-    tt[fy * N + x0 + l] = strip_at<N>(sm, l, fy);
+  fft_regs<N, false>(v, sm + line * S::LS, tt, a.t.tw);
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) {
+    const int fy = tt + S::TPL * r;
+    if (in_rows<N>(fy, out_row0, out_nrow)) tc[fy * N] = v[r];
   }
 }
 
 // ---------------------------------------------------------------- A: E_U pdir, row IFFT
 template <int N>
 __device__ __forceinline__ void task_rows_u_scatter(const DfArgs& a, int slot, int strip, float2* sm) {
-  constexpr int TH = FftCfg<N>::THREADS;
+  using S = Strip<N>;
+  using TH = StripThread<N, false>;
   const DarkDev& L = a.L;
-  const int r0 = strip * kLines;
-  strip_zero<N>(sm);
-  __syncthreads();
+  const int line = TH::line(), tt = TH::t(), row = strip * S::LINES + line;
+  const bool valid = row < L.u_nrow;
+  const int fy = wrapN(L.u_row0 + row, N);
   const float2* pv = a.vec_p + size_t(slot) * a.max_unknown;
-  for (int idx = threadIdx.x; idx < kLines * L.d_ncol; idx += TH) {
-    const int l = idx / L.d_ncol, c = idx % L.d_ncol;
-    if (r0 + l >= L.u_nrow) continue;
-    const int fy = wrapN(L.u_row0 + r0 + l, N);
-    const int e = __ldg(&L.dmap[fy * L.d_ncol + c]);
-    if (e >= 0 && e < L.n_unknown) strip_at<N>(sm, l, wrapN(L.d_col0 + c, N)) = ldcg2(&pv[e]);
+  const int32_t* drow = L.dmap + fy * L.d_ncol;
+  float2 v[S::R];
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) {
+    const int c = col_of<N>(tt + S::TPL * r, L.d_col0);
+    v[r] = make_float2(0.f, 0.f);
+    if (valid && unsigned(c) < unsigned(L.d_ncol)) {
+      const int e = __ldg(&drow[c]);
+      if (unsigned(e) < unsigned(L.n_unknown)) v[r] = ldcg2(&pv[e]);
+    }
   }
-  __syncthreads();
-  fft_lines<N, true>(sm, a.t.tw);
-  float2* tt = a.T + size_t(slot) * (N * N);
-  for (int idx = threadIdx.x; idx < kLines * N; idx += TH) {
-    const int l = idx / N, e = idx % N;
-    if (r0 + l >= L.u_nrow) continue;
-    tt[wrapN(L.u_row0 + r0 + l, N) * N + e] = strip_at<N>(sm, l, e);
+  fft_regs<N, true>(v, sm + line * S::LS, tt, a.t.tw);
+  if (valid) {
+    float2* tr = a.T + size_t(slot) * (N * N) + fy * N;
+#pragma unroll
+    for (int r = 0; r < S::R; ++r) tr[tt + S::TPL * r] = v[r];
   }
 }
 
@@ -239,37 +243,38 @@ __device__ __forceinline__ void task_rows_u_scatter(const DfArgs& a, int slot, i
 template <int N>
 __device__ __forceinline__ void task_rows_u_gather(const DfArgs& a, int slot, int strip, float2* sm, float* red,
                                                    bool with_dot) {
-  constexpr int TH = FftCfg<N>::THREADS;
+  using S = Strip<N>;
+  using TH = StripThread<N, false>;
   const DarkDev& L = a.L;
-  const int r0 = strip * kLines;
-  const float2* tt = a.T + size_t(slot) * (N * N);
-  for (int idx = threadIdx.x; idx < kLines * N; idx += TH) {
-    const int l = idx / N, e = idx % N;
-    float2 v = make_float2(0.f, 0.f);
-    if (r0 + l < L.u_nrow) v = ldcg2(&tt[wrapN(L.u_row0 + r0 + l, N) * N + e]);
-    strip_at<N>(sm, l, e) = v;
-  }
-  __syncthreads();
-  fft_lines<N, false>(sm, a.t.tw);
+  const int line = TH::line(), tt = TH::t(), row = strip * S::LINES + line;
+  const bool valid = row < L.u_nrow;
+  const int fy = wrapN(L.u_row0 + row, N);
+  const float2* tr = a.T + size_t(slot) * (N * N) + fy * N;
+  float2 v[S::R];
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) v[r] = valid ? ldcg2(&tr[tt + S::TPL * r]) : make_float2(0.f, 0.f);
+  fft_regs<N, false>(v, sm + line * S::LS, tt, a.t.tw);
   float2* wv = a.vec_w + size_t(slot) * a.max_unknown;
   const float2* pv = a.vec_p + size_t(slot) * a.max_unknown;
+  const int32_t* drow = L.dmap + fy * L.d_ncol;
   const float scale = 1.f / float(N * N);
   float dot = 0.f;
-  for (int idx = threadIdx.x; idx < kLines * L.d_ncol; idx += TH) {
-    const int l = idx / L.d_ncol, c = idx % L.d_ncol;
-    if (r0 + l >= L.u_nrow) continue;
-    const int fy = wrapN(L.u_row0 + r0 + l, N);
-    const int e = __ldg(&L.dmap[fy * L.d_ncol + c]);
-    if (e >= 0 && e < L.n_unknown) {
-      const float2 w = cscale(strip_at<N>(sm, l, wrapN(L.d_col0 + c, N)), scale);
-      wv[e] = w;
-      if (with_dot) {
-        const float2 p = ldcg2(&pv[e]);
-        dot += p.x * w.x + p.y * w.y;         // Re(conj(p) w)
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) {
+    const int c = col_of<N>(tt + S::TPL * r, L.d_col0);
+    if (valid && unsigned(c) < unsigned(L.d_ncol)) {
+      const int e = __ldg(&drow[c]);
+      if (unsigned(e) < unsigned(L.n_unknown)) {
+        const float2 w = cscale(v[r], scale);
+        wv[e] = w;
+        if (with_dot) {
+          const float2 p = ldcg2(&pv[e]);
+          dot += p.x * w.x + p.y * w.y;         // Re(conj(p) w)
+        }
       }
     }
   }
-  dot = block_sum<TH>(dot, red);
+  dot = block_sum<S::THREADS>(dot, red);
   if (threadIdx.x == 0) a.dot_part[size_t(slot) * a.dot_parts + strip] = dot;
 }
 
@@ -357,10 +362,10 @@ __device__ __forceinline__ bool task_cg_update(const DfArgs& a, int slot, int n_
 enum { PH_BUILD = 0, PH_COLS_P, PH_ROWS_Q, PH_COLS_MUL, PH_COLS_MUL_CONJ, PH_U_GATHER0, PH_U_GATHER, PH_U_SCATTER };
 
 template <int N, int PHASE>
-__global__ void __launch_bounds__(FftCfg<N>::THREADS) df_phase_kernel(DfArgs a, int check_done) {
+__global__ void __launch_bounds__(Strip<N>::THREADS, Strip<N>::MINB) df_phase_kernel(DfArgs a, int check_done) {
   extern __shared__ float2 sm[];
   __shared__ float c_sh[kMaxZern];
-  __shared__ float red[FftCfg<N>::THREADS / 32];
+  __shared__ float red[Strip<N>::THREADS / 32];
   const int slot = blockIdx.y, strip = blockIdx.x;
   const int tile = resolve_tile_idx(a.live, a.live_count, a.chunk0, slot);
   if (tile < 0) return;
@@ -396,8 +401,8 @@ struct Sched {
 };
 
 template <int N>
-__global__ void __launch_bounds__(FftCfg<N>::THREADS, FftCfg<N>::MINB) df_persistent_kernel(DfArgs a, Sched sc) {
-  constexpr int TH = FftCfg<N>::THREADS;
+__global__ void __launch_bounds__(Strip<N>::THREADS, Strip<N>::MINB) df_persistent_kernel(DfArgs a, Sched sc) {
+  constexpr int TH = Strip<N>::THREADS;
   extern __shared__ float2 sm[];
   __shared__ float c_sh[kMaxZern];
   __shared__ float red[TH / 32];
@@ -481,8 +486,9 @@ __global__ void __launch_bounds__(FftCfg<N>::THREADS, FftCfg<N>::MINB) df_persis
 template <int N>
 static void darkfield_led_n(const DevTables& t, const DarkDev& L, int led_pos, int n_dark_used, const Workspace& w,
                             const LaunchCtx& c, const float* d_int, int df_iters, float df_tol, int df_mode) {
-  constexpr int TH = FftCfg<N>::THREADS;
-  constexpr size_t SM = strip_smem_bytes(N);
+  constexpr int TH = Strip<N>::THREADS;
+  constexpr int kLines = Strip<N>::LINES;
+  constexpr size_t SM = Strip<N>::SMEM;
   static bool attr = false;
   static int resident = 0;
   if (!attr) {

@@ -113,127 +113,117 @@ void launch_zero_dead(const DevTables& t, const int32_t* status, int batch, floa
 
 // ---------------------------------------------------------------------------------- S1-S2
 template <int N>
-__global__ void __launch_bounds__(FftCfg<N>::THREADS)
+__global__ void __launch_bounds__(Strip<N>::THREADS, Strip<N>::MINB)
 kk_log_rowfft(DevTables t, const float* __restrict__ d_int, const double* __restrict__ stats, float floor_rel,
               float2* __restrict__ G, const int32_t* __restrict__ live, const int32_t* __restrict__ live_count,
               int chunk0) {
+  using S = Strip<N>;
+  using TH = StripThread<N, false>;
   extern __shared__ float2 sm[];
-  const int slot = blockIdx.z, led = blockIdx.y, row0 = blockIdx.x * kLines;
+  const int slot = blockIdx.z, led = blockIdx.y;
   const int tile = resolve_tile_idx(live, live_count, chunk0, slot);
   if (tile < 0) return;
-  const float* img = d_int + (size_t(tile) * t.n_img + led) * (N * N);
+  const int line = TH::line(), tt = TH::t(), y = blockIdx.x * S::LINES + line;
+  const float* img = d_int + (size_t(tile) * t.n_img + led) * (N * N) + y * N;
   const float mean = float(stats[(size_t(tile) * t.n_img + led) * 3] / double(N * N));
   const float lo = floor_rel * mean;                                   // R6
-  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
-    const int l = idx / N, e = idx % N;
-    const float v = __ldg(&img[(row0 + l) * N + e]);
-    strip_at<N>(sm, l, e) = make_float2(logf(fmaxf(v, lo)), 0.f);     // Re of Eq. 4
-  }
-  __syncthreads();
-  fft_lines<N, false>(sm, t.tw);
-  float2* g = G + (size_t(slot) * t.nb + led) * (N * N);
-  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
-    const int l = idx / N, e = idx % N;
-    g[(row0 + l) * N + e] = strip_at<N>(sm, l, e);
-  }
+  float2 v[S::R];
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) v[r] = make_float2(logf(fmaxf(__ldg(&img[tt + S::TPL * r]), lo)), 0.f);  // Re of Eq. 4
+  fft_regs<N, false>(v, sm + line * S::LS, tt, t.tw);
+  float2* g = G + (size_t(slot) * t.nb + led) * (N * N) + y * N;
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) g[tt + S::TPL * r] = v[r];
 }
 
 // ---------------------------------------------------------------------------------- S2-S4
 template <int N>
-__global__ void __launch_bounds__(FftCfg<N>::THREADS)
+__global__ void __launch_bounds__(Strip<N>::THREADS, Strip<N>::MINB)
 kk_col_mask(DevTables t, float2* __restrict__ G, const int32_t* __restrict__ live_count, int chunk0) {
+  using S = Strip<N>;
+  using TH = StripThread<N, true>;
   extern __shared__ float2 sm[];
-  const int slot = blockIdx.z, led = blockIdx.y, x0 = blockIdx.x * kLines;
+  const int slot = blockIdx.z, led = blockIdx.y;
   if (chunk0 + slot >= *live_count) return;
-  float2* g = G + (size_t(slot) * t.nb + led) * (N * N);
-  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
-    const int l = idx % kLines, e = idx / kLines;
-    strip_at<N>(sm, l, e) = g[e * N + x0 + l];
-  }
-  __syncthreads();
-  fft_lines<N, false>(sm, t.tw);
-  const uint8_t* w2 = t.halfplane2 + size_t(led) * (N * N);
+  const int line = TH::line(), tt = TH::t(), x = blockIdx.x * S::LINES + line;
+  float2* g = G + (size_t(slot) * t.nb + led) * (N * N) + x;
+  float2 v[S::R];
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) v[r] = g[(tt + S::TPL * r) * N];
+  fft_regs<N, false>(v, sm + line * S::LS, tt, t.tw);
+  const uint8_t* w2 = t.halfplane2 + size_t(led) * (N * N) + x;
   const float scale = 0.5f / float(N * N);                              // w = w2/2, and the 1/N^2 of F^-1
-  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
-    const int l = idx % kLines, e = idx / kLines;                       // e = fy, column fx = x0 + l
-    const float w = float(w2[e * N + x0 + l]) * scale;                  // Eq. 5
-    float2& v = strip_at<N>(sm, l, e);
-    v = cscale(v, w);
-  }
-  __syncthreads();
-  fft_lines<N, true>(sm, t.tw);
-  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
-    const int l = idx % kLines, e = idx / kLines;
-    g[e * N + x0 + l] = strip_at<N>(sm, l, e);
-  }
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) v[r] = cscale(v[r], float(__ldg(&w2[(tt + S::TPL * r) * N])) * scale);   // Eq. 5
+  fft_regs<N, true>(v, sm + line * S::LS, tt, t.tw);
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) g[(tt + S::TPL * r) * N] = v[r];
 }
 
 // ---------------------------------------------------------------------------------- S4-S5
 template <int N>
-__global__ void __launch_bounds__(FftCfg<N>::THREADS)
+__global__ void __launch_bounds__(Strip<N>::THREADS, Strip<N>::MINB)
 kk_row_exp(DevTables t, float2* __restrict__ G, const int32_t* __restrict__ live_count, int chunk0) {
+  using S = Strip<N>;
+  using TH = StripThread<N, false>;
   extern __shared__ float2 sm[];
-  const int slot = blockIdx.z, led = blockIdx.y, row0 = blockIdx.x * kLines;
+  const int slot = blockIdx.z, led = blockIdx.y;
   if (chunk0 + slot >= *live_count) return;
-  float2* g = G + (size_t(slot) * t.nb + led) * (N * N);
-  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
-    const int l = idx / N, e = idx % N;
-    strip_at<N>(sm, l, e) = g[(row0 + l) * N + e];
-  }
-  __syncthreads();
-  fft_lines<N, true>(sm, t.tw);
-  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
-    const int l = idx / N, e = idx % N;
-    float2& v = strip_at<N>(sm, l, e);
-    const float a = expf(v.x);                                          // Eq. 6
+  const int line = TH::line(), tt = TH::t(), y = blockIdx.x * S::LINES + line;
+  float2* g = G + (size_t(slot) * t.nb + led) * (N * N) + y * N;
+  float2 v[S::R];
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) v[r] = g[tt + S::TPL * r];
+  fft_regs<N, true>(v, sm + line * S::LS, tt, t.tw);
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) {
+    const float a = expf(v[r].x);                                       // Eq. 6
     float sn, cs;
-    sincosf(v.y, &sn, &cs);
-    v = make_float2(a * cs, a * sn);
+    sincosf(v[r].y, &sn, &cs);
+    v[r] = make_float2(a * cs, a * sn);
   }
-  __syncthreads();
-  fft_lines<N, false>(sm, t.tw);
-  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
-    const int l = idx / N, e = idx % N;
-    g[(row0 + l) * N + e] = strip_at<N>(sm, l, e);
-  }
+  fft_regs<N, false>(v, sm + line * S::LS, tt, t.tw);
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) g[tt + S::TPL * r] = v[r];
 }
 
 // ---------------------------------------------------------------------------------- S5 (Eq. 7)
 template <int N>
-__global__ void __launch_bounds__(FftCfg<N>::THREADS)
-kk_col_gather(DevTables t, const float2* __restrict__ G, float2* __restrict__ S,
+__global__ void __launch_bounds__(Strip<N>::THREADS, Strip<N>::MINB)
+kk_col_gather(DevTables t, const float2* __restrict__ G, float2* __restrict__ Sp,
               const int32_t* __restrict__ live_count, int chunk0) {
+  using S = Strip<N>;
+  using TH = StripThread<N, true>;
   extern __shared__ float2 sm[];
-  const int slot = blockIdx.z, led = blockIdx.y, c0 = blockIdx.x * kLines;
+  const int slot = blockIdx.z, led = blockIdx.y, c0 = blockIdx.x * S::LINES;
   if (chunk0 + slot >= *live_count) return;
   const int ncol = t.bf_ncol[led];
   if (c0 >= ncol) return;
-  const int col0 = t.bf_col0[led];
-  const float2* g = G + (size_t(slot) * t.nb + led) * (N * N);
-  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
-    const int l = idx % kLines, e = idx / kLines;
-    float2 v = make_float2(0.f, 0.f);
-    if (c0 + l < ncol) v = g[e * N + ((col0 + c0 + l + N) & (N - 1))];
-    strip_at<N>(sm, l, e) = v;
-  }
-  __syncthreads();
-  fft_lines<N, false>(sm, t.tw);
-  const int32_t* map = t.bf_map + t.bf_map_off[led];
-  float2* s = S + size_t(slot) * t.disc_total;
+  const int line = TH::line(), tt = TH::t(), c = c0 + line;
+  const bool valid = c < ncol;
+  const int fx = (t.bf_col0[led] + c + N) & (N - 1);
+  const float2* g = G + (size_t(slot) * t.nb + led) * (N * N) + fx;
+  float2 v[S::R];
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) v[r] = valid ? g[(tt + S::TPL * r) * N] : make_float2(0.f, 0.f);
+  fft_regs<N, false>(v, sm + line * S::LS, tt, t.tw);
+  if (!valid) return;
+  const int32_t* map = t.bf_map + t.bf_map_off[led] + c;
+  float2* s = Sp + size_t(slot) * t.disc_total;
   const float scale = 1.f / float(N * N);
-  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
-    const int l = idx % kLines, e = idx / kLines;
-    if (c0 + l >= ncol) continue;
-    const int ent = map[e * ncol + c0 + l];
-    if (ent >= 0) s[ent] = cscale(strip_at<N>(sm, l, e), scale);
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) {
+    const int ent = __ldg(&map[(tt + S::TPL * r) * ncol]);
+    if (ent >= 0) s[ent] = cscale(v[r], scale);
   }
 }
 
 template <int N>
 static void launch_kk_n(const DevTables& t, const Workspace& w, const LaunchCtx& c, const float* d_int,
                         const double* stats, float floor_rel) {
-  constexpr int TH = FftCfg<N>::THREADS;
-  constexpr size_t SM = strip_smem_bytes(N);
+  using S = Strip<N>;
+  constexpr int TH = S::THREADS;
+  constexpr size_t SM = S::SMEM;
   static bool attr = false;
   if (!attr) {
     cudaFuncSetAttribute(kk_log_rowfft<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
@@ -242,14 +232,14 @@ static void launch_kk_n(const DevTables& t, const Workspace& w, const LaunchCtx&
     cudaFuncSetAttribute(kk_col_gather<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
     attr = true;
   }
-  dim3 grid(N / kLines, t.nb, c.chunk_tiles);
+  dim3 grid(N / S::LINES, t.nb, c.chunk_tiles);
   { ProfScope ps(c, CAT_KK_LOG_ROWFFT);
     kk_log_rowfft<N><<<grid, TH, SM, c.stream>>>(t, d_int, stats, floor_rel, w.G, c.live, c.live_count, c.chunk0); }
   { ProfScope ps(c, CAT_KK_COL_MASK);
     kk_col_mask<N><<<grid, TH, SM, c.stream>>>(t, w.G, c.live_count, c.chunk0); }
   { ProfScope ps(c, CAT_KK_ROW_EXP);
     kk_row_exp<N><<<grid, TH, SM, c.stream>>>(t, w.G, c.live_count, c.chunk0); }
-  dim3 grid4((t.bf_max_ncol + kLines - 1) / kLines, t.nb, c.chunk_tiles);
+  dim3 grid4((t.bf_max_ncol + S::LINES - 1) / S::LINES, t.nb, c.chunk_tiles);
   { ProfScope ps(c, CAT_KK_COL_GATHER);
     kk_col_gather<N><<<grid4, TH, SM, c.stream>>>(t, w.G, w.S, c.live_count, c.chunk0); }
 }
@@ -266,33 +256,34 @@ void launch_kk(const DevTables& t, const Workspace& w, const LaunchCtx& c, const
 
 // ---------------------------------------------------------------------------------- plain 2-D FFT
 template <int N, bool INV, bool COLS>
-__global__ void __launch_bounds__(FftCfg<N>::THREADS) fft_pass_kernel(float2* __restrict__ d, const float2* __restrict__ tw) {
+__global__ void __launch_bounds__(Strip<N>::THREADS, Strip<N>::MINB)
+fft_pass_kernel(float2* __restrict__ d, const float2* __restrict__ tw) {
+  using S = Strip<N>;
+  using TH = StripThread<N, COLS>;
   extern __shared__ float2 sm[];
-  float2* g = d + size_t(blockIdx.y) * (N * N);
-  const int s0 = blockIdx.x * kLines;
-  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
-    if (COLS) { const int l = idx % kLines, e = idx / kLines; strip_at<N>(sm, l, e) = g[e * N + s0 + l]; }
-    else      { const int l = idx / N, e = idx % N;           strip_at<N>(sm, l, e) = g[(s0 + l) * N + e]; }
-  }
-  __syncthreads();
-  fft_lines<N, INV>(sm, tw);
-  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
-    if (COLS) { const int l = idx % kLines, e = idx / kLines; g[e * N + s0 + l] = strip_at<N>(sm, l, e); }
-    else      { const int l = idx / N, e = idx % N;           g[(s0 + l) * N + e] = strip_at<N>(sm, l, e); }
-  }
+  const int line = TH::line(), tt = TH::t(), l = blockIdx.x * S::LINES + line;
+  float2* g = d + size_t(blockIdx.y) * (N * N) + (COLS ? l : l * N);
+  constexpr int STR = COLS ? N : 1;
+  float2 v[S::R];
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) v[r] = g[(tt + S::TPL * r) * STR];
+  fft_regs<N, INV>(v, sm + line * S::LS, tt, tw);
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) g[(tt + S::TPL * r) * STR] = v[r];
 }
 
 template <int N>
 static int fft2d_n(float2* d, int batch, bool inverse, const float2* tw, cudaStream_t s) {
-  constexpr int TH = FftCfg<N>::THREADS;
-  constexpr size_t SM = strip_smem_bytes(N);
+  using S = Strip<N>;
+  constexpr int TH = S::THREADS;
+  constexpr size_t SM = S::SMEM;
   cudaFuncSetAttribute(fft_pass_kernel<N, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
   cudaFuncSetAttribute(fft_pass_kernel<N, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
   cudaFuncSetAttribute(fft_pass_kernel<N, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
   cudaFuncSetAttribute(fft_pass_kernel<N, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
   for (int b0 = 0; b0 < batch; b0 += 32768) {
     const int nb = batch - b0 < 32768 ? batch - b0 : 32768;
-    dim3 grid(N / kLines, nb);
+    dim3 grid(N / S::LINES, nb);
     float2* p = d + size_t(b0) * (N * N);
     if (inverse) {
       fft_pass_kernel<N, true, false><<<grid, TH, SM, s>>>(p, tw);

@@ -13,56 +13,59 @@ namespace apic {
 __device__ __forceinline__ int wrapNo(int k, int n) { return (k + n) & (n - 1); }
 
 template <int N>
-__global__ void __launch_bounds__(FftCfg<N>::THREADS)
+__global__ void __launch_bounds__(Strip<N>::THREADS, Strip<N>::MINB)
 out_rows(DevTables t, const float2* __restrict__ O, float2* __restrict__ TOUT,
          const int32_t* __restrict__ live_count, int chunk0) {
+  using S = Strip<N>;
+  using TH = StripThread<N, false>;
   extern __shared__ float2 sm[];
-  const int slot = blockIdx.z, ax = blockIdx.y, r0 = blockIdx.x * kLines;
+  const int slot = blockIdx.z, ax = blockIdx.y;
   if (chunk0 + slot >= *live_count) return;
-  const float2* o = O + size_t(slot) * (N * N);
+  const int line = TH::line(), tt = TH::t(), row = blockIdx.x * S::LINES + line;
+  const bool valid = row < t.known_nrow;
+  const int fy = wrapNo(t.known_row0 + row, N);
+  const float2* o = O + size_t(slot) * (N * N) + fy * N;
   const float2* ramp = t.ramp + ax * N;
-  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
-    const int l = idx / N, e = idx % N;
-    float2 v = make_float2(0.f, 0.f);
-    if (r0 + l < t.known_nrow) v = cmul(o[wrapNo(t.known_row0 + r0 + l, N) * N + e], __ldg(&ramp[e]));
-    strip_at<N>(sm, l, e) = v;
+  float2 v[S::R];
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) {
+    const int fx = tt + S::TPL * r;
+    v[r] = valid ? cmul(o[fx], __ldg(&ramp[fx])) : make_float2(0.f, 0.f);
   }
-  __syncthreads();
-  fft_lines<N, true>(sm, t.tw);
+  fft_regs<N, true>(v, sm + line * S::LS, tt, t.tw);
+  if (!valid) return;
   const int on = N * t.u;
-  float2* to = TOUT + size_t(slot) * N * on;
-  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
-    const int l = idx / N, e = idx % N;
-    if (r0 + l >= t.known_nrow) continue;
-    to[size_t(wrapNo(t.known_row0 + r0 + l, N)) * on + e * t.u + ax] = strip_at<N>(sm, l, e);
-  }
+  float2* to = TOUT + (size_t(slot) * N + fy) * on + ax;
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) to[(tt + S::TPL * r) * t.u] = v[r];
 }
 
 template <int N>
-__global__ void __launch_bounds__(FftCfg<N>::THREADS)
+__global__ void __launch_bounds__(Strip<N>::THREADS, Strip<N>::MINB)
 out_cols(DevTables t, const float2* __restrict__ TOUT, float2* __restrict__ field,
          const int32_t* __restrict__ live, const int32_t* __restrict__ live_count, int chunk0) {
+  using S = Strip<N>;
+  using TH = StripThread<N, true>;
   extern __shared__ float2 sm[];
-  const int slot = blockIdx.z, ay = blockIdx.y, x0 = blockIdx.x * kLines;
+  const int slot = blockIdx.z, ay = blockIdx.y;
   const int tile = resolve_tile_idx(live, live_count, chunk0, slot);
   if (tile < 0) return;
+  const int line = TH::line(), tt = TH::t(), x = blockIdx.x * S::LINES + line;
   const int on = N * t.u;
-  const float2* to = TOUT + size_t(slot) * N * on;
+  const float2* to = TOUT + size_t(slot) * N * on + x;
   const float2* ramp = t.ramp + ay * N;
-  strip_zero<N>(sm);
-  __syncthreads();
-  for (int idx = threadIdx.x; idx < kLines * t.known_nrow; idx += FftCfg<N>::THREADS) {
-    const int l = idx % kLines, r = idx / kLines;
-    const int fy = wrapNo(t.known_row0 + r, N);
-    strip_at<N>(sm, l, fy) = cmul(to[size_t(fy) * on + x0 + l], __ldg(&ramp[fy]));
+  float2 v[S::R];
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) {
+    const int fy = tt + S::TPL * r;
+    const int ky = fy < N / 2 ? fy : fy - N;
+    v[r] = (unsigned(ky - t.known_row0) < unsigned(t.known_nrow)) ? cmul(to[size_t(fy) * on], __ldg(&ramp[fy]))
+                                                                  : make_float2(0.f, 0.f);
   }
-  __syncthreads();
-  fft_lines<N, true>(sm, t.tw);
-  float2* f = field + size_t(tile) * on * on;
-  for (int idx = threadIdx.x; idx < kLines * N; idx += FftCfg<N>::THREADS) {
-    const int l = idx % kLines, e = idx / kLines;
-    f[size_t(e * t.u + ay) * on + x0 + l] = strip_at<N>(sm, l, e);
-  }
+  fft_regs<N, true>(v, sm + line * S::LS, tt, t.tw);
+  float2* f = field + size_t(tile) * on * on + x;
+#pragma unroll
+  for (int r = 0; r < S::R; ++r) f[size_t((tt + S::TPL * r) * t.u + ay) * on] = v[r];
 }
 
 __global__ void __launch_bounds__(256) pupil_kernel(DevTables t, const float* __restrict__ coef,
@@ -86,8 +89,9 @@ __global__ void __launch_bounds__(256) pupil_kernel(DevTables t, const float* __
 
 template <int N>
 static void output_n(const DevTables& t, const Workspace& w, const LaunchCtx& c, float* d_field) {
-  constexpr int TH = FftCfg<N>::THREADS;
-  constexpr size_t SM = strip_smem_bytes(N);
+  using S = Strip<N>;
+  constexpr int TH = S::THREADS, kLines = S::LINES;
+  constexpr size_t SM = S::SMEM;
   static bool attr = false;
   if (!attr) {
     cudaFuncSetAttribute(out_rows<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));

@@ -12,7 +12,7 @@ namespace apic {
 
 struct DevTables {
   int n, u, nb, nd, nz, n_img;   // n_img = nb + nd
-  const float2* tw;              // [N] e^{-2 pi i m / N}
+  const float2* tw;              // twiddle tables of fft_core.cuh (build_twiddles)
   // NA-matching side
   const uint8_t* halfplane2;     // [nb][N*N] FFT order, 2*w of Eq. 5
   int disc_total;                // sum_i |D_i|

@@ -120,8 +120,10 @@ def test_config2_full_size_bench_configuration(A):
     tiles = list(range(64))
     stacks, truths = make_batch(cfg, tiles)
     plan, field, zern, pupil, status = gpu_reconstruct(A, cfg, stacks)
-    assert plan.info["chunk_tiles"] < 64              # several internal passes
     assert np.all(status == 0)
+    # the same batch in three balanced internal passes (22 + 21 + 21 tiles) gives the same bits
+    _, field3, zern3, _, _ = gpu_reconstruct(A, cfg, stacks, chunk_tiles=24)
+    assert np.array_equal(field, field3) and np.array_equal(zern, zern3)
     sample = [0, 37, 63]
     refs, _ = oracle_reconstruct(cfg, stacks[sample])
     for ref, b in zip(refs, sample):
