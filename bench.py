@@ -45,7 +45,8 @@ def parse_args():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (2 = default workload)")
     ap.add_argument("--tiles", type=int, default=0, help="tiles per step and per GPU (0 = the config's batch, capped at 64)")
     ap.add_argument("--chunk", type=int, default=0, help="apic_params.chunk_tiles (0 = library default)")
-    ap.add_argument("--df-mode", type=int, default=0, help="darkfield scheduler: 0 persistent task kernel, 1 launch per phase")
+    ap.add_argument("--df-mode", type=int, default=0, help="darkfield scheduler: 0 team kernel, 1 launch per phase, 2 ticket kernel")
+    ap.add_argument("--df-team", type=int, default=0, help="apic_params.df_team: CTAs per tile of the team kernel (0 = auto)")
     ap.add_argument("--df-tol", type=float, default=-1.0, help="CG tolerance (default: the library's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -199,7 +200,7 @@ def main():
     host = np.concatenate([stacks] * reps)[:tiles]
     x = torch.from_numpy(host).cuda()
     popts = {"df_tol": args.df_tol} if args.df_tol > 0 else {}
-    plan = A.Plan.from_config(cfg, max_batch=tiles, chunk_tiles=args.chunk, df_mode=args.df_mode, **popts)
+    plan = A.Plan.from_config(cfg, max_batch=tiles, chunk_tiles=args.chunk, df_mode=args.df_mode, df_team=args.df_team, **popts)
     n, on, nz = cfg.tile_n, cfg.out_n, plan.nz
     out = (torch.empty((tiles, on, on), dtype=torch.complex64, device="cuda"),
            torch.empty((tiles, nz), dtype=torch.float32, device="cuda"),
@@ -220,7 +221,7 @@ def main():
         vis = os.environ["CUDA_VISIBLE_DEVICES"].split(",")
         sampler.gpu_id = vis[local] if local < len(vis) else str(local)
     sampler.start()
-    plan.profile_begin(stride=1 if args.df_mode == 0 else 4, max_samples=16384)
+    plan.profile_begin(stride=1 if args.df_mode != 1 else 4, max_samples=16384)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches = 0
     barrier()
@@ -248,7 +249,7 @@ def main():
     sms = torch.cuda.get_device_properties(local).multi_processor_count
     peak = sms * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     total_kernel_ms = sum(v[0] / max(v[1], 1) * v[2] for v in prof.values())
-    dominant = "df_persistent" if args.df_mode == 0 and cfg.n_dark else "df_cols_mul"
+    dominant = "df_persistent" if args.df_mode != 1 and cfg.n_dark else "df_cols_mul"
     if not cfg.n_dark:
         dominant = max(prof, key=lambda k: prof[k][0] / max(prof[k][1], 1) * prof[k][2])
     ms_sum, samples, nlaunch = prof[dominant]

@@ -74,9 +74,13 @@ typedef struct {
                             min(max_batch, internal chunk)                                       */
   int chunk_tiles;       /* tiles per internal pass; 0 = chosen so that one pass's transform
                             working set stays inside the 126 MB L2                              */
-  int df_mode;           /* darkfield scheduler: 0 = persistent task kernel (one launch per LED and
-                            pass, stops when every tile has converged), 1 = one launch per phase
-                            (df_iters iterations are always enqueued)                            */
+  int df_mode;           /* darkfield scheduler: 0 = team kernel (one launch per pass covers every
+                            darkfield LED; a cluster of df_team CTAs owns a tile and meets at
+                            cluster barriers between phases), 1 = one launch per phase (df_iters
+                            iterations are always enqueued), 2 = ticket-scheduled persistent task
+                            kernel (one launch per LED and pass)                               */
+  int df_team;           /* df_mode 0: CTAs (= SMs) per tile, 1 | 2 | 4 | 8; 0 = chosen from the
+                            pass size (as many as the pass leaves SMs for)                      */
 } apic_params;
 
 /* Fills *p with the defaults (kk_pad 1, refine_iters 3, df_iters 48, df_tol 1e-5, floor 1e-6,

@@ -38,7 +38,7 @@ class ApicParams(C.Structure):
                 ("n_zernike", C.c_int), ("noll", C.POINTER(C.c_int)), ("kk_pad", C.c_int),
                 ("refine_iters", C.c_int), ("df_iters", C.c_int), ("df_tol", C.c_float),
                 ("intensity_floor", C.c_float), ("bg_mode", C.c_int), ("bg_threshold", C.c_float),
-                ("max_batch", C.c_int), ("chunk_tiles", C.c_int), ("df_mode", C.c_int)]
+                ("max_batch", C.c_int), ("chunk_tiles", C.c_int), ("df_mode", C.c_int), ("df_team", C.c_int)]
 
 
 class PlanInfo(C.Structure):

@@ -30,6 +30,7 @@ struct apic_plan {
   HostTables host;
   DevTables dev{};
   std::vector<DarkDev> dark;
+  const DarkDev* d_dark = nullptr;   // device copy of `dark` (team kernel)
   Workspace ws{};
   BatchState bs{};
   std::vector<void*> allocs;
@@ -96,6 +97,7 @@ void apic_params_default(apic_params* p) {
   p->max_batch = 64;
   p->chunk_tiles = 0;
   p->df_mode = 0;
+  p->df_team = 0;
 }
 
 const char* apic_strerror(int err) {
@@ -214,6 +216,7 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
     max_unknown = std::max(max_unknown, L.n_unknown);
     dot_parts = std::max(dot_parts, (L.u_nrow + strip_lines(n) - 1) / strip_lines(n));
   }
+  ok = ok && plan->upload(&plan->d_dark, plan->dark);
   // ---- workspace
   Workspace& w = plan->ws;
   const size_t nn = size_t(n) * n;
@@ -321,9 +324,12 @@ int apic_reconstruct(apic_plan* plan, const float* d_intensity, int batch, float
     launch_kk(t, w, c, d_intensity, plan->bs.stats, p.intensity_floor);                       // S1-S5
     launch_aberration(t, w, c, p.refine_iters, d_zernike, d_status);                          // S6
     launch_stitch(t, w, c);                                                                   // S7
-    for (int k = 0; k < n_dark_used; ++k)                                                     // S8-S10
-      launch_darkfield_led(t, plan->dark[k], k, std::max(1, n_dark_used), w, c, d_intensity, p.df_iters, p.df_tol,
-                           p.df_mode);
+    if (p.df_mode == 0)                                                                       // S8-S10
+      launch_darkfield_team(t, plan->d_dark, n_dark_used, w, c, d_intensity, p.df_iters, p.df_tol, p.df_team);
+    else
+      for (int k = 0; k < n_dark_used; ++k)
+        launch_darkfield_led(t, plan->dark[k], k, std::max(1, n_dark_used), w, c, d_intensity, p.df_iters, p.df_tol,
+                             p.df_mode);
     launch_output(t, w, c, d_field, d_pupil);                                                 // S10
   }
   if (!cuda_ok(cudaGetLastError(), "apic_reconstruct launch")) return APIC_ECUDA;

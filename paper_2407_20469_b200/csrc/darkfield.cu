@@ -521,7 +521,7 @@ static void darkfield_led_n(const DevTables& t, const DarkDev& L, int led_pos, i
   a.live = c.live; a.live_count = c.live_count; a.chunk0 = c.chunk0; a.n_tiles = B; a.sync = w.df_sync; a.work = w.df_work;
   const int n_d = strips(L.d_nrow), n_q = strips(L.q_nrow), n_u = strips(L.u_nrow), n_c = N / kLines;
 
-  if (df_mode == 0) {
+  if (df_mode == 2) {
     Sched sc{};
     const int n[12] = {n_d, n_c, n_q, n_c, n_u, 1, n_u, n_c, n_q, n_c, n_u, 1};
     sc.cum[0] = 0;

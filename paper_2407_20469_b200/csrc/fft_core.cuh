@@ -128,10 +128,11 @@ template <> struct FftCfg<128> { static constexpr int R = 4,  B = 8, LINES = 8, 
 template <> struct FftCfg<256> { static constexpr int R = 16, B = 1, LINES = 16, MINB = 4; };
 template <> struct FftCfg<512> { static constexpr int R = 8,  B = 8, LINES = 8,  MINB = 2; };
 
-template <int N>
+// LINES_ lines per strip (default: the per-N value of FftCfg; the darkfield team kernel uses wider strips)
+template <int N, int LINES_ = FftCfg<N>::LINES>
 struct Strip {
   using C = FftCfg<N>;
-  static constexpr int R = C::R, B = C::B, LINES = C::LINES, MINB = C::MINB;
+  static constexpr int R = C::R, B = C::B, LINES = LINES_, MINB = C::MINB;
   static constexpr int TPL = N / R;                 // threads per line
   static constexpr int THREADS = LINES * TPL;
   static constexpr int LS = N + N / 16 + 1;         // padded line stride (odd)
@@ -179,29 +180,31 @@ __device__ __forceinline__ int pad16(int i) { return i + (i >> 4); }
 
 // Thread -> (line, t) inside a strip.  Row strips: t fastest (a half-warp reads 128 contiguous
 // bytes of one row).  Column strips: line fastest (LINES consecutive columns of one row).
-template <int N, bool COLS>
+template <int N, bool COLS, int LINES_ = FftCfg<N>::LINES>
 struct StripThread {
-  using S = Strip<N>;
+  using S = Strip<N, LINES_>;
   static __device__ __forceinline__ int line() { return COLS ? int(threadIdx.x) % S::LINES : int(threadIdx.x) / S::TPL; }
   static __device__ __forceinline__ int t() { return COLS ? int(threadIdx.x) / S::LINES : int(threadIdx.x) % S::TPL; }
 };
 
 // In: v[r] = x[t + TPL r].  Out: v[r] = X[t + TPL r].  `ln` = this thread's line in shared memory.
-// Contains barriers: every thread of the CTA must call it.
-template <int N, bool INV>
+// Contains barriers: every thread of the CTA must call it.  TW_SMEM: `tw` points to a copy of the
+// twiddle table in shared memory (plain loads) instead of global memory (read-only path).
+template <int N, bool INV, bool TW_SMEM = false>
 __device__ __forceinline__ void fft_regs(float2 (&v)[Strip<N>::R], float2* __restrict__ ln, int t,
                                          const float2* __restrict__ tw) {
   using S = Strip<N>;
+  auto twl = [&](int i) { return TW_SMEM ? tw[i] : __ldg(&tw[i]); };
   constexpr int R = S::R, B = S::B, TPL = S::TPL;
   // ---- step 1: DFT_R over n3, twiddle
   RegDft<R, INV>::run(v);
   if (B == 1) {
 #pragma unroll
-    for (int k1 = 1; k1 < R; ++k1) v[k1] = twmul<INV>(v[k1], __ldg(&tw[k1 * R + t]));
+    for (int k1 = 1; k1 < R; ++k1) v[k1] = twmul<INV>(v[k1], twl(k1 * R + t));
   } else {
     const int n2 = t / R;
 #pragma unroll
-    for (int k1 = 1; k1 < R; ++k1) v[k1] = twmul<INV>(v[k1], __ldg(&tw[k1 * B + n2]));
+    for (int k1 = 1; k1 < R; ++k1) v[k1] = twmul<INV>(v[k1], twl(k1 * B + n2));
   }
   __syncthreads();                                   // earlier readers of this line are done
 #pragma unroll
@@ -218,7 +221,7 @@ __device__ __forceinline__ void fft_regs(float2 (&v)[Strip<N>::R], float2* __res
       RegDft<(B > 1 ? B : 4), INV>::run(u);
 #pragma unroll
       for (int k2 = 0; k2 < B; ++k2) {
-        u[k2] = twmul<INV>(u[k2], __ldg(&tw[R * B + k2 * PAIRS + t]));
+        u[k2] = twmul<INV>(u[k2], twl(R * B + k2 * PAIRS + t));
         ln[pad16(n1 + R * k2 + R * B * k1)] = u[k2];     // same positions this thread read
       }
     }

@@ -123,7 +123,10 @@ bool build_geometry(const apic_params& p, HostTables& t, std::string& err) {
   if (p.df_iters < 1) { err = "df_iters must be >= 1"; return false; }
   if (p.bg_mode < 0 || p.bg_mode > 2) { err = "bg_mode must be 0, 1 or 2"; return false; }
   if (p.max_batch < 1) { err = "max_batch must be >= 1"; return false; }
-  if (p.df_mode < 0 || p.df_mode > 1) { err = "df_mode must be 0 (persistent) or 1 (multi-launch)"; return false; }
+  if (p.df_mode < 0 || p.df_mode > 2) { err = "df_mode must be 0 (team kernel), 1 (multi-launch) or 2 (ticket kernel)"; return false; }
+  if (!(p.df_team == 0 || p.df_team == 1 || p.df_team == 2 || p.df_team == 4 || p.df_team == 8)) {
+    err = "df_team must be 0 (auto), 1, 2, 4 or 8"; return false;
+  }
   for (int a = 0; a < p.n_zernike; ++a) {
     if (p.noll[a] < 4) { err = "Noll indices must be >= 4 (piston/tilt are the null space of Eq. 10)"; return false; }
     for (int b = 0; b < a; ++b)

@@ -154,6 +154,9 @@ void launch_stitch(const DevTables& t, const Workspace& w, const LaunchCtx& c);
 // darkfield (S8-S10) for one LED
 void launch_darkfield_led(const DevTables& t, const DarkDev& L, int led_pos, int n_dark_used, const Workspace& w,
                           const LaunchCtx& c, const float* d_int, int df_iters, float df_tol, int df_mode);
+// darkfield (S8-S10), every LED in one launch (df_team.cu)
+void launch_darkfield_team(const DevTables& t, const DarkDev* d_leds, int n_leds, const Workspace& w, const LaunchCtx& c,
+                           const float* d_int, int df_iters, float df_tol, int team_size);
 // outputs
 void launch_output(const DevTables& t, const Workspace& w, const LaunchCtx& c, float* d_field, float* d_pupil);
 

@@ -87,7 +87,7 @@ def test_single_tile_configs(A, index):
 
 
 # ---------------------------------------------------------------------------------- config 2
-@pytest.mark.parametrize("df_mode", [0, 1])
+@pytest.mark.parametrize("df_mode", [0, 1, 2])
 def test_config2_reduced_all_tiles_ragged_chunks(A, df_mode):
     """64x64 variant of config 2 (8 + 16 LEDs, Poisson noise, 3x grid): every tile against the
     oracle, with 5 tiles over chunks of 2 (two full chunks and a ragged tail); both darkfield
@@ -103,7 +103,7 @@ def test_config2_reduced_all_tiles_ragged_chunks(A, df_mode):
     assert its.min() >= 1 and its.max() < 48          # CG converged by its tolerance, not the cap
 
 
-@pytest.mark.parametrize("df_mode", [0, 1])
+@pytest.mark.parametrize("df_mode", [0, 1, 2])
 def test_config2_128(A, df_mode):
     cfg = get_config(2, tile_n=128, batch=3, grid=(2, 2))
     stacks, _ = make_batch(cfg, range(3))
@@ -215,8 +215,14 @@ def test_results_are_bit_reproducible_and_batch_invariant(A):
     assert np.array_equal(f1, f2) and np.array_equal(z1, z2)
     _, f3, z3, _, _ = gpu_reconstruct(A, cfg, stacks[::-1].copy(), chunk_tiles=3)
     assert np.array_equal(f1, f3[::-1]) and np.array_equal(z1, z3[::-1])
-    _, f4, z4, _, _ = gpu_reconstruct(A, cfg, stacks, df_mode=1)      # the other scheduler: same arithmetic
-    assert np.array_equal(f1, f4) and np.array_equal(z1, z4)
+    for team in (1, 2, 4):                                            # team size does not change the arithmetic
+        _, ft, zt, _, _ = gpu_reconstruct(A, cfg, stacks, df_team=team)
+        assert np.array_equal(f1, ft) and np.array_equal(z1, zt), team
+    _, f4, z4, _, _ = gpu_reconstruct(A, cfg, stacks, df_mode=1)      # the launch-per-phase and the ticket
+    _, f5, z5, _, _ = gpu_reconstruct(A, cfg, stacks, df_mode=2)      # schedulers share their task bodies
+    assert np.array_equal(f4, f5) and np.array_equal(z4, z5)
+    # the team kernel sums the CG dot products in a different order: same result within fp32 rounding
+    assert np.linalg.norm(f1 - f4) <= 1e-5 * np.linalg.norm(f4) and np.array_equal(z1, z4)
 
 
 def test_host_entry_point_and_batch_limits(A):
