@@ -83,7 +83,7 @@ typedef struct {
                             pass size (as many as the pass leaves SMs for)                      */
 } apic_params;
 
-/* Fills *p with the defaults (kk_pad 1, refine_iters 3, df_iters 48, df_tol 1e-5, floor 1e-6,
+/* Fills *p with the defaults (kk_pad 1, refine_iters 3, df_iters 48, df_tol 1e-4, floor 1e-6,
  * bg off, max_batch 64); the caller then sets the geometry fields. */
 void apic_params_default(apic_params* p);
 

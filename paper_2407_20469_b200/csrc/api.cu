@@ -90,7 +90,7 @@ void apic_params_default(apic_params* p) {
   p->kk_pad = 1;
   p->refine_iters = 3;
   p->df_iters = 48;
-  p->df_tol = 1e-5f;
+  p->df_tol = 1e-4f;
   p->intensity_floor = 1e-6f;
   p->bg_mode = 0;
   p->bg_threshold = 0.f;
