@@ -45,7 +45,7 @@ def parse_args():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (2 = default workload)")
     ap.add_argument("--tiles", type=int, default=0, help="tiles per step and per GPU (0 = the config's batch, capped at 64)")
     ap.add_argument("--chunk", type=int, default=0, help="apic_params.chunk_tiles (0 = library default)")
-    ap.add_argument("--df-mode", type=int, default=0, help="darkfield scheduler: 0 team kernel, 1 launch per phase, 2 ticket kernel")
+    ap.add_argument("--df-mode", type=int, default=0, help="darkfield scheduler: 0 team kernel (reduced grids at N=256), 1 launch per phase, 2 ticket kernel, 3 team kernel on the full grid")
     ap.add_argument("--df-team", type=int, default=0, help="apic_params.df_team: CTAs per tile of the team kernel (0 = auto)")
     ap.add_argument("--df-tol", type=float, default=-1.0, help="CG tolerance (default: the library's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -255,10 +255,12 @@ def main():
     ms_sum, samples, nlaunch = prof[dominant]
     avg_ms = ms_sum / max(samples, 1)
     if dominant == "df_persistent":
-        # executed work counted by the kernel itself: N-point line transforms of all its strip tasks
-        lines = plan.profile_work()
-        flop_per_launch = lines * fft_line / max(nlaunch, 1)
-        note = f"{lines} executed {n}-point line FFTs x 5 N log2 N over {nlaunch} launches (pointwise work not counted)"
+        # executed work counted by the kernel itself: 5 L log2 L per L-point line transform of its strip tasks
+        # (L = N, or the per-LED reduced grid sizes 96..256 of df_mgrid.cu at N = 256)
+        flop = plan.profile_work()
+        flop_per_launch = flop / max(nlaunch, 1)
+        note = (f"{flop:.4g} nominal FFT flop executed (5 L log2 L per L-point line transform, counted by the kernel) "
+                f"over {nlaunch} launches; pointwise work not counted")
     elif dominant == "df_cols_mul":
         n_chunks = -(-tiles // chunk)
         flop_per_launch = (2 * n * fft_line + 6.0 * n * n) * tiles / n_chunks

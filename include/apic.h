@@ -78,7 +78,9 @@ typedef struct {
                             darkfield LED; a cluster of df_team CTAs owns a tile and meets at
                             cluster barriers between phases), 1 = one launch per phase (df_iters
                             iterations are always enqueued), 2 = ticket-scheduled persistent task
-                            kernel (one launch per LED and pass)                               */
+                            kernel (one launch per LED and pass), 3 = team kernel on the full
+                            N x N grid.  At N = 256 mode 0 runs the CG mat-vecs on per-LED
+                            reduced cyclic grids; other N: same as 3     */
   int df_team;           /* df_mode 0: CTAs (= SMs) per tile, 1 | 2 | 4 | 8; 0 = chosen from the
                             pass size (as many as the pass leaves SMs for)                      */
 } apic_params;
@@ -118,6 +120,9 @@ int apic_plan_info(const apic_plan* plan, apic_plan_info_t* info);
  * receive up to `cap` darkfield index-set sizes in processing order.  Used by the CPU tests. */
 int apic_geometry_info(const apic_params* p, apic_plan_info_t* info, int* led, int* n_unknown,
                        int* n_equations, int cap);
+/* Host only: the reduced cyclic grid (mx, my) chosen for each used darkfield LED, in processing
+ * order (alias-free iff mx, my exceed the extent of U - P - Q per axis). */
+int apic_geometry_dark_grids(const apic_params* p, int* mx, int* my, int cap);
 
 /* Darkfield index-set sizes in processing order (ascending |kappa|, ties by input order):
  * led[k] = input index, n_unknown[k] = |U|, n_equations[k] = |Q|.  Arrays hold n_dark_used ints. */
@@ -161,6 +166,13 @@ int apic_debug_copy(const apic_plan* plan, int which, void* d_dst, int tiles, vo
  * unnormalised e^{+j..}.  n in {64,128,256,512}. */
 int apic_fft2d(float* d_data, int n, int batch, int inverse, void* cuda_stream);
 
+/* The mixed-radix line transforms of the darkfield solver's reduced cyclic grids (lengths 16*R1,
+ * R1 in {6,8,10,12,16}), exposed for kernel-level parity tests: d_data
+ * [batch][my][mx] complex64 in place, mx, my in {96,128,160,192,256}.  mode 0 / 1: forward /
+ * inverse 2-D DFT (unnormalised) by the "type X" transform; mode 2 / 3: per axis X inverse then
+ * Y forward (2), or X forward then Y inverse (3), divided by the length: the identity. */
+int apic_fft2d_xy(float* d_data, int mx, int my, int batch, int mode, void* cuda_stream);
+
 /* Number of kernels launched by the last apic_reconstruct on this plan (bench's gpu_launches). */
 int apic_last_launch_count(const apic_plan* plan);
 
@@ -174,9 +186,10 @@ int apic_profile_categories(void);
 const char* apic_profile_category_name(int cat);
 int apic_profile_begin(apic_plan* plan, int stride, int max_samples);
 int apic_profile_end(apic_plan* plan, double* ms_sum, long long* samples, long long* launches);
-/* Number of N-point line transforms executed by the persistent darkfield kernels since
- * apic_profile_begin (synchronises the device). */
-int apic_profile_work(apic_plan* plan, unsigned long long* line_transforms);
+/* Nominal FFT flop (5 L log2 L per executed L-point line transform, counted by the kernels
+ * themselves) of the persistent darkfield kernels since apic_profile_begin (synchronises the
+ * device). */
+int apic_profile_work(apic_plan* plan, unsigned long long* fft_flop);
 
 const char* apic_strerror(int err);
 const char* apic_last_cuda_error(void);

@@ -21,8 +21,8 @@ TILE_OK, TILE_BACKGROUND, TILE_BAD_INPUT, TILE_SOLVE_FAILED = 0, 1, 2, 3
 DBG_SUBSPECTRA, DBG_OBJECT_SPECTRUM, DBG_DF_ITERS = 0, 1, 2
 
 EXPORTS = ("apic_params_default", "apic_plan_create", "apic_plan_destroy", "apic_plan_info",
-           "apic_geometry_info", "apic_plan_dark_sets", "apic_reconstruct", "apic_reconstruct_host",
-           "apic_debug_buffer", "apic_debug_copy", "apic_fft2d", "apic_last_launch_count", "apic_strerror",
+           "apic_geometry_info", "apic_geometry_dark_grids", "apic_plan_dark_sets", "apic_reconstruct", "apic_reconstruct_host",
+           "apic_debug_buffer", "apic_debug_copy", "apic_fft2d", "apic_fft2d_xy", "apic_last_launch_count", "apic_strerror",
            "apic_last_cuda_error", "apic_version", "apic_profile_categories", "apic_profile_category_name",
            "apic_profile_begin", "apic_profile_end", "apic_profile_work")
 
@@ -71,6 +71,7 @@ def load() -> C.CDLL:
     lib.apic_plan_info.argtypes = [C.c_void_p, C.POINTER(PlanInfo)]
     lib.apic_geometry_info.argtypes = [C.POINTER(ApicParams), C.POINTER(PlanInfo), C.POINTER(C.c_int),
                                        C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_int]
+    lib.apic_geometry_dark_grids.argtypes = [C.POINTER(ApicParams), C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_int]
     lib.apic_plan_dark_sets.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int)]
     lib.apic_reconstruct.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
                                      C.c_void_p, C.c_void_p]
@@ -78,6 +79,7 @@ def load() -> C.CDLL:
     lib.apic_debug_buffer.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)]
     lib.apic_debug_copy.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p]
     lib.apic_fft2d.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
+    lib.apic_fft2d_xy.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p]
     lib.apic_last_launch_count.argtypes = [C.c_void_p]
     for name in ("apic_strerror", "apic_last_cuda_error", "apic_version"):
         getattr(lib, name).restype = C.c_char_p
@@ -134,6 +136,15 @@ def geometry_info(params: ApicParams, max_dark: int = 256):
     _check(lib.apic_geometry_info(C.byref(params), C.byref(info), led, nu, nq, max_dark), "apic_geometry_info")
     n = min(info.n_dark_used, max_dark)
     return info.as_dict(), [(led[i], nu[i], nq[i]) for i in range(n)]
+
+
+def geometry_dark_grids(params: ApicParams, max_dark: int = 256):
+    """Host-only: [(mx, my), ...] reduced cyclic grids of the used darkfield LEDs, processing order."""
+    lib = load()
+    info, dark = geometry_info(params, max_dark)
+    mx, my = (C.c_int * max_dark)(), (C.c_int * max_dark)()
+    _check(lib.apic_geometry_dark_grids(C.byref(params), mx, my, max_dark), "apic_geometry_dark_grids")
+    return [(mx[i], my[i]) for i in range(len(dark))]
 
 
 class Plan:
@@ -254,4 +265,17 @@ def fft2d(x, inverse: bool = False):
     lib = load()
     stream = torch.cuda.current_stream(x.device).cuda_stream
     _check(lib.apic_fft2d(x.data_ptr(), x.shape[1], x.shape[0], int(inverse), C.c_void_p(stream)), "apic_fft2d")
+    return x
+
+
+def fft2d_xy(x, mode: int = 0):
+    """In-place batched transform of a complex64 CUDA tensor [B][my][mx] by the reduced-grid line
+    FFTs (apic_fft2d_xy: mode 0 forward, 1 inverse, 2 / 3 X-then-Y identity round trips)."""
+    import torch
+    if not (x.is_cuda and x.dtype == torch.complex64 and x.is_contiguous() and x.dim() == 3):
+        raise ApicError("x must be a contiguous complex64 CUDA tensor [B][my][mx]")
+    lib = load()
+    stream = torch.cuda.current_stream(x.device).cuda_stream
+    _check(lib.apic_fft2d_xy(x.data_ptr(), x.shape[2], x.shape[1], x.shape[0], int(mode), C.c_void_p(stream)),
+           "apic_fft2d_xy")
     return x

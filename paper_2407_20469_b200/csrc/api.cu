@@ -8,6 +8,7 @@
 
 #include "../../include/apic.h"
 #include "fft_core.cuh"
+#include "fft_xy.cuh"
 #include "plan.hpp"
 
 using namespace apic;
@@ -129,6 +130,18 @@ int apic_geometry_info(const apic_params* p, apic_plan_info_t* info, int* led, i
   return APIC_OK;
 }
 
+int apic_geometry_dark_grids(const apic_params* p, int* mx, int* my, int cap) {
+  if (!p || !mx || !my) return APIC_EINVAL;
+  HostTables h;
+  std::string err;
+  if (!build_geometry(*p, h, err)) { g_plan_err = err; return APIC_EINVAL; }
+  for (int k = 0; k < int(h.dark.size()) && k < cap; ++k) {
+    mx[k] = h.dark[k].mx;
+    my[k] = h.dark[k].my;
+  }
+  return APIC_OK;
+}
+
 int apic_plan_destroy(apic_plan* plan) {
   if (!plan) return APIC_OK;
   for (void* q : plan->allocs) cudaFree(q);
@@ -168,6 +181,12 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
     std::vector<float2> tw;
     build_twiddles(n, tw);
     ok = ok && plan->upload(&d.tw, tw);
+    std::vector<float2> txy, one;
+    for (int r1 : {6, 8, 10, 12, 16}) {
+      build_twiddles_xy(r1, one);
+      txy.insert(txy.end(), one.begin(), one.end());
+    }
+    ok = ok && plan->upload(&d.tw_xy, txy);
     std::vector<float2> ramp(size_t(h.u) * n);
     for (int a = 0; a < h.u; ++a)
       for (int f = 0; f < n; ++f) {
@@ -211,6 +230,9 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
     ok = ok && plan->upload(&q.zern, L.zern);
     ok = ok && plan->upload(&q.dmap, L.dmap);
     ok = ok && plan->upload(&q.qmap, L.qmap);
+    q.mx = L.mx; q.my = L.my;
+    ok = ok && plan->upload(&q.dmap_m, L.dmap_m);
+    ok = ok && plan->upload(&q.qmask_m, L.qmask_m);
     plan->dark.push_back(q);
     max_eq = std::max(max_eq, L.n_eq);
     max_unknown = std::max(max_unknown, L.n_unknown);
@@ -243,6 +265,7 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
   ok = ok && plan->dalloc(&w.O, c * nn, false);
   ok = ok && plan->dalloc(&w.T, c * nn, false);
   ok = ok && plan->dalloc(&w.PF, c * nn, false);
+  ok = ok && plan->dalloc(&w.TM, c * (h.dark.empty() ? 1 : nn), false);
   ok = ok && plan->dalloc(&w.vec_d, c * max_eq, false);
   ok = ok && plan->dalloc(&w.vec_x, c * max_unknown, false);
   ok = ok && plan->dalloc(&w.vec_s, c * max_unknown, false);
@@ -324,7 +347,9 @@ int apic_reconstruct(apic_plan* plan, const float* d_intensity, int batch, float
     launch_kk(t, w, c, d_intensity, plan->bs.stats, p.intensity_floor);                       // S1-S5
     launch_aberration(t, w, c, p.refine_iters, d_zernike, d_status);                          // S6
     launch_stitch(t, w, c);                                                                   // S7
-    if (p.df_mode == 0)                                                                       // S8-S10
+    if (p.df_mode == 0 && t.n == 256)                                                         // S8-S10
+      launch_darkfield_mgrid(t, plan->d_dark, n_dark_used, w, c, d_intensity, p.df_iters, p.df_tol, p.df_team);
+    else if (p.df_mode == 0 || p.df_mode == 3)
       launch_darkfield_team(t, plan->d_dark, n_dark_used, w, c, d_intensity, p.df_iters, p.df_tol, p.df_team);
     else
       for (int k = 0; k < n_dark_used; ++k)
@@ -410,6 +435,25 @@ int apic_fft2d(float* d_data, int n, int batch, int inverse, void* cuda_stream) 
   }
   launch_fft2d(reinterpret_cast<float2*>(d_data), n, batch, inverse != 0, tw_cache[slot], static_cast<cudaStream_t>(cuda_stream));
   if (!cuda_ok(cudaGetLastError(), "apic_fft2d")) return APIC_ECUDA;
+  return APIC_OK;
+}
+
+int apic_fft2d_xy(float* d_data, int mx, int my, int batch, int mode, void* cuda_stream) {
+  auto okl = [](int l) { return l == 96 || l == 128 || l == 160 || l == 192 || l == 256; };
+  if (!d_data || batch < 1 || !okl(mx) || !okl(my) || mode < 0 || mode > 3) return APIC_EINVAL;
+  static float2* tw = nullptr;
+  if (!tw) {
+    std::vector<float2> txy, one;
+    for (int r1 : {6, 8, 10, 12, 16}) {
+      build_twiddles_xy(r1, one);
+      txy.insert(txy.end(), one.begin(), one.end());
+    }
+    if (!cuda_ok(cudaMalloc(reinterpret_cast<void**>(&tw), txy.size() * sizeof(float2)), "cudaMalloc")) return APIC_ECUDA;
+    if (!cuda_ok(cudaMemcpy(tw, txy.data(), txy.size() * sizeof(float2), cudaMemcpyHostToDevice), "cudaMemcpy")) return APIC_ECUDA;
+  }
+  if (launch_fft2d_xy(reinterpret_cast<float2*>(d_data), mx, my, batch, mode, tw, static_cast<cudaStream_t>(cuda_stream)))
+    return APIC_EINVAL;
+  if (!cuda_ok(cudaGetLastError(), "apic_fft2d_xy")) return APIC_ECUDA;
   return APIC_OK;
 }
 

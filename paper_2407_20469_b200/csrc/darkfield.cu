@@ -49,7 +49,7 @@ struct DfArgs {
   int chunk0, n_tiles;
   // persistent scheduler state: [0] ticket, [1] tiles finished, [2 + slot] per-tile progress
   int32_t* sync;
-  unsigned long long* work;   // executed line transforms (for the roofline line of bench.py)
+  unsigned long long* work;   // executed nominal flop, 5 N log2 N per line transform (roofline line of bench.py)
 };
 
 __device__ __forceinline__ int wrapN(int k, int n) { return (k + n) & (n - 1); }
@@ -478,7 +478,7 @@ __global__ void __launch_bounds__(Strip<N>::THREADS, Strip<N>::MINB) df_persiste
         atomicAdd(&a.sync[1], 1);
       }
       atomicAdd(&a.sync[2 + slot], 1);
-      if (sc.lines[ph]) atomicAdd(a.work, (unsigned long long)sc.lines[ph]);
+      if (sc.lines[ph]) atomicAdd(a.work, (unsigned long long)sc.lines[ph] * (unsigned long long)(5 * N * (31 - __clz(N))));
     }
   }
 }

@@ -475,7 +475,8 @@ __global__ void __launch_bounds__(Strip<N, TeamCfg<N>::LINES>::THREADS, TeamCfg<
       team_sync(multi);                                    // O complete before the next LED reads it
     }
   }
-  if (threadIdx.x == 0 && lines) atomicAdd(a.work, lines);
+  // reported as nominal flop: 5 N log2 N per N-point line transform
+  if (threadIdx.x == 0 && lines) atomicAdd(a.work, lines * (unsigned long long)(5 * N * (31 - __clz(N))));
 }
 
 template <int N>

@@ -123,7 +123,7 @@ bool build_geometry(const apic_params& p, HostTables& t, std::string& err) {
   if (p.df_iters < 1) { err = "df_iters must be >= 1"; return false; }
   if (p.bg_mode < 0 || p.bg_mode > 2) { err = "bg_mode must be 0, 1 or 2"; return false; }
   if (p.max_batch < 1) { err = "max_batch must be >= 1"; return false; }
-  if (p.df_mode < 0 || p.df_mode > 2) { err = "df_mode must be 0 (team kernel), 1 (multi-launch) or 2 (ticket kernel)"; return false; }
+  if (p.df_mode < 0 || p.df_mode > 3) { err = "df_mode must be 0 (team kernel), 1 (multi-launch), 2 (ticket kernel) or 3 (full-grid team kernel)"; return false; }
   if (!(p.df_team == 0 || p.df_team == 1 || p.df_team == 2 || p.df_team == 4 || p.df_team == 8)) {
     err = "df_team must be 0 (auto), 1, 2, 4 or 8"; return false;
   }
@@ -360,6 +360,35 @@ bool build_geometry(const apic_params& p, HostTables& t, std::string& err) {
         int fy = ((iy - h) + n) % n;
         L.qmap[size_t(fy) * L.q_ncol + (ix - h - L.q_col0)] = mq++;
       }
+    {
+      // reduced cyclic grid: per axis the lags u - p - k (u in U, p in P, k in Q) must stay inside (-m, m)
+      int pc0, pnc, pr0, pnr;
+      bbox(P, pc0, pnc, pr0, pnr);
+      auto extent = [](int u0, int un, int p0, int pn, int q0, int qn) {
+        const int hi = (u0 + un - 1) - p0 - q0, lo = u0 - (p0 + pn - 1) - (q0 + qn - 1);
+        return std::max(std::abs(hi), std::abs(lo));
+      };
+      const int ex = extent(L.u_col0, L.u_ncol, pc0, pnc, L.q_col0, L.q_ncol);
+      const int ey = extent(L.u_row0, L.u_nrow, pr0, pnr, L.q_row0, L.q_nrow);
+      auto pick = [&](int e) {
+        const int cand[5] = {3 * n / 8, n / 2, 5 * n / 8, 3 * n / 4, n};
+        for (int c : cand)
+          if (c > e && c >= L.d_ncol && c >= L.d_nrow) return c;
+        return n;
+      };
+      L.mx = pick(ex); L.my = pick(ey);
+      L.dmap_m.assign(size_t(L.mx) * L.my, -1);
+      L.qmask_m.assign(size_t(L.mx) * L.my, 0);
+      auto pos = [&](int kx, int ky) {
+        return size_t(((ky % L.my) + L.my) % L.my) * L.mx + size_t(((kx % L.mx) + L.mx) % L.mx);
+      };
+      for (int iy = 0; iy < n; ++iy)
+        for (int ix = 0; ix < n; ++ix) {
+          const size_t q = size_t(iy) * n + ix;
+          if (d.v[q]) L.dmap_m[pos(ix - h, iy - h)] = ent[q];
+          if (Q.v[q]) L.qmask_m[pos(ix - h, iy - h)] = 1;
+        }
+    }
     for (size_t q = 0; q < size_t(n) * n; ++q) known.v[q] |= U.v[q];
     t.dark.push_back(std::move(L));
   }

@@ -31,6 +31,12 @@ struct DarkLed {
   std::vector<int32_t> dmap;   // [N (fy)][d_ncol] -> disc entry or -1
   std::vector<int32_t> qmap;   // [N (fy)][q_ncol] -> equation index or -1
   double unknown_fraction = 0;
+  // Reduced cyclic grid (df_mgrid.cu): the mat-vecs of Eq. 13 only need correlations at lags in Q, so a
+  // cyclic grid of mx x my bins is alias-free as soon as mx, my exceed the extent of U - P - Q per axis.
+  // mx, my in {3N/8, N/2, 5N/8, 3N/4, N}; bin (kx, ky) sits at ((ky mod my) * mx + (kx mod mx)).
+  int mx = 0, my = 0;
+  std::vector<int32_t> dmap_m; // [my][mx] -> disc entry or -1
+  std::vector<uint8_t> qmask_m;// [my][mx] -> 1 on Q
 };
 
 struct HostTables {

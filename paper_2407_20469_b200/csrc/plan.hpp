@@ -13,6 +13,7 @@ namespace apic {
 struct DevTables {
   int n, u, nb, nd, nz, n_img;   // n_img = nb + nd
   const float2* tw;              // twiddle tables of fft_core.cuh (build_twiddles)
+  const float2* tw_xy;           // [5][256] twiddles of fft_xy.cuh for R1 = 6, 8, 10, 12, 16 (N = 256 only)
   // NA-matching side
   const uint8_t* halfplane2;     // [nb][N*N] FFT order, 2*w of Eq. 5
   int disc_total;                // sum_i |D_i|
@@ -50,6 +51,9 @@ struct DarkDev {
   const int32_t* dmap;                  // [N(fy)][d_ncol] -> disc entry | -1
   const int32_t* qmap;                  // [N(fy)][q_ncol] -> equation | -1
   int led;                              // input index among the darkfield LEDs
+  int mx, my;                           // reduced cyclic grid of the CG mat-vecs (geometry.hpp)
+  const int32_t* dmap_m;                // [my][mx] -> disc entry | -1
+  const uint8_t* qmask_m;               // [my][mx] -> 1 on Q
 };
 
 constexpr int kGramRows = 512;          // rows per Gram partial (aberration kernels)
@@ -67,6 +71,7 @@ struct Workspace {
   float2* O;               // [chunk][N*N] object spectrum, FFT order
   float2* T;               // [chunk][N*N] transform scratch
   float2* PF;              // [chunk][N*N] p = F^-1 P_hat of the current darkfield LED
+  float2* TM;              // [chunk][N*N] transform scratch on the reduced grid (df_mgrid.cu)
   float2* vec_d;           // [chunk][max_eq]
   float2* vec_x;           // [chunk][max_unknown]
   float2* vec_s;
@@ -78,7 +83,7 @@ struct Workspace {
   int32_t* cg_done;        // [chunk]
   int32_t* cg_iters;       // [chunk][n_dark_used]
   int32_t* df_sync;        // [2 + chunk] persistent scheduler: ticket, finished tiles, per-tile progress
-  unsigned long long* df_work;   // [1] line transforms executed by the persistent darkfield kernels
+  unsigned long long* df_work;   // [1] nominal flop (5 L log2 L per L-point line transform) executed by the darkfield kernels
   float2* TOUT;            // [chunk][N][uN]
   int max_eq, max_unknown;
 };
@@ -157,6 +162,10 @@ void launch_darkfield_led(const DevTables& t, const DarkDev& L, int led_pos, int
 // darkfield (S8-S10), every LED in one launch (df_team.cu)
 void launch_darkfield_team(const DevTables& t, const DarkDev* d_leds, int n_leds, const Workspace& w, const LaunchCtx& c,
                            const float* d_int, int df_iters, float df_tol, int team_size);
+// darkfield (S8-S10) on reduced cyclic grids, every LED in one launch (df_mgrid.cu; N = 256)
+void launch_darkfield_mgrid(const DevTables& t, const DarkDev* d_leds, int n_leds, const Workspace& w, const LaunchCtx& c,
+                            const float* d_int, int df_iters, float df_tol, int team_size);
+int launch_fft2d_xy(float2* d, int mx, int my, int batch, int mode, const float2* tw_xy, cudaStream_t s);
 // outputs
 void launch_output(const DevTables& t, const Workspace& w, const LaunchCtx& c, float* d_field, float* d_pupil);
 

@@ -70,6 +70,23 @@ def test_fft2d_matches_oracle_transform(A, n):
 
 
 # ---------------------------------------------------------------------------------- configs 0, 1
+
+@pytest.mark.parametrize("mx,my", [(96, 160), (160, 128), (192, 96), (128, 256), (256, 192)])
+def test_reduced_grid_line_transforms(A, mx, my):
+    """fft_xy.cuh (lengths 16*R1, R1 in {6,8,10,12,16}) against the DFT: type X alone as a 2-D
+    transform (forward and inverse), and X followed by Y as the identity."""
+    import torch
+    rng = np.random.default_rng(mx * 1000 + my)
+    x = (rng.standard_normal((3, my, mx)) + 1j * rng.standard_normal((3, my, mx))).astype(np.complex64)
+    for mode in (0, 1):
+        y = A.fft2d_xy(torch.from_numpy(x.copy()).cuda(), mode).cpu().numpy()
+        ref = np.fft.fft2(x.astype(np.complex128)) if mode == 0 else np.fft.ifft2(x.astype(np.complex128)) * (mx * my)
+        assert rel_l2(y, ref) < 2e-6, (mx, my, mode)
+    for mode in (2, 3):
+        y = A.fft2d_xy(torch.from_numpy(x.copy()).cuda(), mode).cpu().numpy()
+        assert rel_l2(y, x) < 2e-6, (mx, my, mode)
+
+
 @pytest.mark.parametrize("index", [0, 1])
 def test_single_tile_configs(A, index):
     cfg = get_config(index)
@@ -124,6 +141,12 @@ def test_config2_full_size_bench_configuration(A):
     # the same batch in three balanced internal passes (22 + 21 + 21 tiles) gives the same bits
     _, field3, zern3, _, _ = gpu_reconstruct(A, cfg, stacks, chunk_tiles=24)
     assert np.array_equal(field, field3) and np.array_equal(zern, zern3)
+    # the darkfield solver on the full N x N grid (df_mode 3) solves the same least-squares problems as the
+    # default reduced cyclic grids: both stop at the same CG tolerance, so they agree far inside the parity bar
+    _, field_full, zern_full, _, _ = gpu_reconstruct(A, cfg, stacks[:8], df_mode=3)
+    assert np.array_equal(zern_full, zern[:8])
+    for b in range(8):
+        assert rel_l2(field[b], field_full[b]) < 2e-5, b
     sample = [0, 37, 63]
     refs, _ = oracle_reconstruct(cfg, stacks[sample])
     for ref, b in zip(refs, sample):
