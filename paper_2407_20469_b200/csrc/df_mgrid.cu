@@ -105,23 +105,37 @@ __device__ __forceinline__ void with_r1(int r1, F&& f) {
   }
 }
 
-// Shared-memory state of a CTA
+// Shared-memory layout of a CTA (all dynamic, so that every access is an LDS/STS and no generic LD/ST):
+//   [bufA kXyBuf][bufB kXyBuf][twx 256][twy 256][tw256 256][misc 128][xs mu][ss mu][ps mu]   (float2 units)
+// misc: Zernike coefficients of the tile (64 floats), block_sum scratch (8 floats), the current DarkDev.
 struct Ctx {
-  float2 *bufA, *bufB;         // exchange buffers [kXyBuf]
-  const float2 *twx, *twy;     // twiddles of the current LED's row (mx) and column (my) lengths
-  const float2* tw256;         // N-grid twiddles
-  float2 *xs, *ss, *ps;        // CG vectors [max_unknown]
-  float* c_sh;
-  float* red;
-  const DarkDev* L;
+  int mu;   // max_unknown
+  __device__ __forceinline__ float2* base() const {
+    extern __shared__ float2 dyn[];
+    return dyn;
+  }
+  __device__ __forceinline__ float2* bufA() const { return base(); }
+  __device__ __forceinline__ float2* bufB() const { return base() + kXyBuf; }
+  __device__ __forceinline__ float2* twx() const { return base() + 2 * kXyBuf; }
+  __device__ __forceinline__ float2* twy() const { return base() + 2 * kXyBuf + 256; }
+  __device__ __forceinline__ float2* tw256() const { return base() + 2 * kXyBuf + 512; }
+  __device__ __forceinline__ float* c_sh() const { return reinterpret_cast<float*>(base() + 2 * kXyBuf + 768); }
+  __device__ __forceinline__ float* red() const { return c_sh() + 64; }
+  __device__ __forceinline__ DarkDev* Lp() const { return reinterpret_cast<DarkDev*>(c_sh() + 80); }
+  __device__ __forceinline__ float2* xs() const { return base() + 2 * kXyBuf + 768 + 128; }
+  __device__ __forceinline__ float2* ss() const { return xs() + mu; }
+  __device__ __forceinline__ float2* ps() const { return ss() + mu; }
 };
+constexpr int kSmFixed = 2 * kXyBuf + 768 + 128;   // float2 entries before the CG vectors
+static_assert(sizeof(DarkDev) <= (256 - 80) * sizeof(float), "DarkDev does not fit the misc region");
+static_assert(kMaxZern <= 64, "c_sh region");
 
 // ================================================================ reduced-grid phases
 // A: E_U pdir (shared memory) -> row IFFT_mx -> TM rows of U
 template <int R1>
 __device__ __noinline__ void ph_rows_u_scatter(const Args& a, const Ctx& c, int slot, unsigned g, unsigned G) {
   using M = XY<R1, false>;
-  const DarkDev& L = *c.L;
+  const DarkDev& L = *c.Lp();
   constexpr int mx = 16 * R1;
   const int my = L.my, n_st = (L.u_nrow + 15) >> 4;
   float2* tm = a.TM + size_t(slot) * (N * N);
@@ -136,11 +150,11 @@ __device__ __noinline__ void ph_rows_u_scatter(const Args& a, const Ctx& c, int 
         v[r] = make_float2(0.f, 0.f);
         if (row < L.u_nrow) {
           const int e = __ldg(&drow[t + 16 * r]);
-          if (unsigned(e) < unsigned(L.n_unknown)) v[r] = c.ps[e];
+          if (unsigned(e) < unsigned(L.n_unknown)) v[r] = c.ps()[e];
         }
       }
     }
-    fft_x<R1, true, false>(v, par ? c.bufB : c.bufA, c.twx);
+    fft_x<R1, true, false>(v, par ? c.bufB() : c.bufA(), c.twx());
     if (M::b_active()) {
       const int row = st * 16 + M::b_line(), k1 = M::b_k1();
       if (row < L.u_nrow) {
@@ -156,7 +170,7 @@ __device__ __noinline__ void ph_rows_u_scatter(const Args& a, const Ctx& c, int 
 template <int R1>
 __device__ __noinline__ void ph_rows_u_gather(const Args& a, const Ctx& c, int slot, unsigned g, unsigned G) {
   using M = XY<R1, false>;
-  const DarkDev& L = *c.L;
+  const DarkDev& L = *c.Lp();
   constexpr int mx = 16 * R1;
   const int my = L.my, n_st = (L.u_nrow + 15) >> 4;
   const float scale = 1.f / float(mx * my);
@@ -171,7 +185,7 @@ __device__ __noinline__ void ph_rows_u_gather(const Args& a, const Ctx& c, int s
 #pragma unroll
       for (int r = 0; r < R1; ++r) v[r] = row < L.u_nrow ? __ldcg(&tr[16 * r]) : make_float2(0.f, 0.f);
     }
-    fft_x<R1, false, false>(v, par ? c.bufB : c.bufA, c.twx);
+    fft_x<R1, false, false>(v, par ? c.bufB() : c.bufA(), c.twx());
     if (M::b_active()) {
       const int row = st * 16 + M::b_line(), k1 = M::b_k1();
       if (row < L.u_nrow) {
@@ -190,7 +204,7 @@ __device__ __noinline__ void ph_rows_u_gather(const Args& a, const Ctx& c, int s
 template <int R1>
 __device__ __noinline__ void ph_rows_q(const Args& a, const Ctx& c, int slot, unsigned g, unsigned G) {
   using M = XY<R1, false>;
-  const DarkDev& L = *c.L;
+  const DarkDev& L = *c.Lp();
   constexpr int mx = 16 * R1;
   const int my = L.my, n_st = (L.q_nrow + 15) >> 4;
   const float scale = 1.f / float(mx * my);
@@ -210,10 +224,10 @@ __device__ __noinline__ void ph_rows_q(const Args& a, const Ctx& c, int slot, un
         for (int k2 = 0; k2 < 16; ++k2) keep |= unsigned(__ldg(&qrow[R1 * k2]) != 0) << k2;
       }
     }
-    fft_x<R1, false, false>(v, c.bufA, c.twx);
+    fft_x<R1, false, false>(v, c.bufA(), c.twx());
 #pragma unroll
     for (int k2 = 0; k2 < 16; ++k2) v[k2] = (keep >> k2 & 1u) ? cscale(v[k2], scale) : make_float2(0.f, 0.f);
-    fft_y<R1, true, false>(v, c.bufB, c.twx);
+    fft_y<R1, true, false>(v, c.bufB(), c.twx());
     if (rowa < L.q_nrow) {
 #pragma unroll
       for (int r = 0; r < R1; ++r) tr[16 * r] = v[r];
@@ -225,7 +239,7 @@ __device__ __noinline__ void ph_rows_q(const Args& a, const Ctx& c, int slot, un
 template <int R1, bool CONJ>
 __device__ __noinline__ void ph_cols_mul(const Args& a, const Ctx& c, int slot, unsigned g, unsigned G) {
   using M = XY<R1, true>;
-  const DarkDev& L = *c.L;
+  const DarkDev& L = *c.Lp();
   constexpr int my = 16 * R1;
   const int mx = L.mx, n_st = mx >> 4;
   const int in0 = modp(CONJ ? L.u_row0 : L.q_row0, my), in_n = CONJ ? L.u_nrow : L.q_nrow;
@@ -245,12 +259,12 @@ __device__ __noinline__ void ph_cols_mul(const Args& a, const Ctx& c, int slot, 
 #pragma unroll
       for (int k2 = 0; k2 < 16; ++k2) p[k2] = __ldcg(&pc[(R1 * k2) * mx]);
     }
-    fft_x<R1, true, true>(v, c.bufA, c.twy);
+    fft_x<R1, true, true>(v, c.bufA(), c.twy());
     if (M::b_active()) {
 #pragma unroll
       for (int k2 = 0; k2 < 16; ++k2) v[k2] = CONJ ? cmulc(v[k2], p[k2]) : cmul(v[k2], p[k2]);
     }
-    fft_y<R1, false, true>(v, c.bufB, c.twy);
+    fft_y<R1, false, true>(v, c.bufB(), c.twy());
 #pragma unroll
     for (int r = 0; r < R1; ++r) {
       const int gy = t + 16 * r;
@@ -263,8 +277,8 @@ __device__ __noinline__ void ph_cols_mul(const Args& a, const Ctx& c, int slot, 
 __device__ __forceinline__ int wrapN(int k) { return (k + N) & (N - 1); }
 __device__ __forceinline__ float2 p_hat_entry(const Args& a, const Ctx& c, const float2* __restrict__ o, int e) {
   // P_hat(k) = O_hat(k) e^{+j phi(k + kappa)} on P = D_i ∩ known
-  const DarkDev& L = *c.L;
-  const float phi = zern_phase(L.zern + size_t(e) * a.t.nz, c.c_sh, a.t.nz);
+  const DarkDev& L = *c.Lp();
+  const float phi = zern_phase(L.zern + size_t(e) * a.t.nz, c.c_sh(), a.t.nz);
   float sn, cs;
   sincosf(phi, &sn, &cs);
   return cmul(__ldcg(&o[__ldg(&L.disc_f[e])]), make_float2(cs, sn));
@@ -272,7 +286,7 @@ __device__ __forceinline__ float2 p_hat_entry(const Args& a, const Ctx& c, const
 
 // P0 (N grid): P_hat rows -> row IFFT_N -> T
 __device__ __noinline__ void ph_build_p_rows_n(const Args& a, const Ctx& c, int slot, unsigned g, unsigned G) {
-  const DarkDev& L = *c.L;
+  const DarkDev& L = *c.Lp();
   const int line = int(threadIdx.x) >> 4, tt = int(threadIdx.x) & 15;
   const int n_st = (L.d_nrow + 15) >> 4;
   const float2* o = a.O + size_t(slot) * (N * N);
@@ -290,7 +304,7 @@ __device__ __noinline__ void ph_build_p_rows_n(const Args& a, const Ctx& c, int 
         if (e >= L.n_unknown) v[r] = p_hat_entry(a, c, o, e);
       }
     }
-    fft_regs<N, true, true>(v, c.bufA + line * S256::LS, tt, c.tw256);
+    fft_regs<N, true, true>(v, c.bufA() + line * S256::LS, tt, c.tw256());
     if (valid) {
       float2* tr = a.T + size_t(slot) * (N * N) + fy * N;
 #pragma unroll
@@ -303,7 +317,7 @@ __device__ __noinline__ void ph_build_p_rows_n(const Args& a, const Ctx& c, int 
 template <int R1>
 __device__ __noinline__ void ph_build_p_rows_m(const Args& a, const Ctx& c, int slot, unsigned g, unsigned G) {
   using M = XY<R1, false>;
-  const DarkDev& L = *c.L;
+  const DarkDev& L = *c.Lp();
   constexpr int mx = 16 * R1;
   const int my = L.my, n_st = (L.d_nrow + 15) >> 4;
   const float2* o = a.O + size_t(slot) * (N * N);
@@ -324,7 +338,7 @@ __device__ __noinline__ void ph_build_p_rows_m(const Args& a, const Ctx& c, int 
         }
       }
     }
-    fft_x<R1, true, false>(v, par ? c.bufB : c.bufA, c.twx);
+    fft_x<R1, true, false>(v, par ? c.bufB() : c.bufA(), c.twx());
     if (M::b_active()) {
       const int row = st * 16 + M::b_line(), k1 = M::b_k1();
       if (row < L.d_nrow) {
@@ -338,7 +352,7 @@ __device__ __noinline__ void ph_build_p_rows_m(const Args& a, const Ctx& c, int 
 
 // P1 (N grid): column IFFT_N -> p_N; I - |p_N|^2; column FFT_N -> T rows of Q
 __device__ __noinline__ void ph_cols_rhs_n(const Args& a, const Ctx& c, int slot, int tile, unsigned g, unsigned G) {
-  const DarkDev& L = *c.L;
+  const DarkDev& L = *c.Lp();
   const int line = int(threadIdx.x) & 15, tt = int(threadIdx.x) >> 4;
   const float* img0 = a.d_int + (size_t(tile) * a.t.n_img + a.t.nb + L.led) * (N * N);
   __syncthreads();
@@ -353,10 +367,10 @@ __device__ __noinline__ void ph_cols_rhs_n(const Args& a, const Ctx& c, int slot
       v[r] = unsigned(ky - L.d_row0) < unsigned(L.d_nrow) ? __ldcg(&tc[fy * N]) : make_float2(0.f, 0.f);
       im[r] = __ldg(&img0[fy * N + x]);
     }
-    fft_regs<N, true, true>(v, c.bufA + line * S256::LS, tt, c.tw256);
+    fft_regs<N, true, true>(v, c.bufA() + line * S256::LS, tt, c.tw256());
 #pragma unroll
     for (int r = 0; r < 16; ++r) v[r] = make_float2(im[r] - (v[r].x * v[r].x + v[r].y * v[r].y), 0.f);   // Eq. 13 lhs, spatial
-    fft_regs<N, false, true>(v, c.bufA + line * S256::LS, tt, c.tw256);
+    fft_regs<N, false, true>(v, c.bufA() + line * S256::LS, tt, c.tw256());
 #pragma unroll
     for (int r = 0; r < 16; ++r) {
       const int fy = tt + 16 * r, ky = fy < N / 2 ? fy : fy - N;
@@ -369,7 +383,7 @@ __device__ __noinline__ void ph_cols_rhs_n(const Args& a, const Ctx& c, int slot
 template <int R1>
 __device__ __noinline__ void ph_cols_pm(const Args& a, const Ctx& c, int slot, unsigned g, unsigned G) {
   using M = XY<R1, true>;
-  const DarkDev& L = *c.L;
+  const DarkDev& L = *c.Lp();
   constexpr int my = 16 * R1;
   const int mx = L.mx, n_st = mx >> 4, d0 = modp(L.d_row0, my);
   const float2* tm = a.TM + size_t(slot) * (N * N);
@@ -384,7 +398,7 @@ __device__ __noinline__ void ph_cols_pm(const Args& a, const Ctx& c, int slot, u
       const int gy = t + 16 * r;
       v[r] = row_in(gy, d0, L.d_nrow, my) ? __ldcg(&tm[gy * mx + x]) : make_float2(0.f, 0.f);
     }
-    fft_x<R1, true, true>(v, par ? c.bufB : c.bufA, c.twy);
+    fft_x<R1, true, true>(v, par ? c.bufB() : c.bufA(), c.twy());
     if (M::b_active()) {
       float2* pc = pf + M::b_k1() * mx + x;
 #pragma unroll
@@ -397,7 +411,7 @@ __device__ __noinline__ void ph_cols_pm(const Args& a, const Ctx& c, int slot, u
 template <int R1>
 __device__ __noinline__ void ph_rows_rhs(const Args& a, const Ctx& c, int slot, unsigned g, unsigned G) {
   using M = XY<R1, false>;
-  const DarkDev& L = *c.L;
+  const DarkDev& L = *c.Lp();
   constexpr int mx = 16 * R1;
   const int my = L.my, n_st = (L.q_nrow + 15) >> 4;
   const int line = int(threadIdx.x) >> 4, tt = int(threadIdx.x) & 15;
@@ -412,7 +426,7 @@ __device__ __noinline__ void ph_rows_rhs(const Args& a, const Ctx& c, int slot, 
     float2 v[16];
 #pragma unroll
     for (int r = 0; r < 16; ++r) v[r] = valid ? __ldcg(&tb[fy * N + tt + 16 * r]) : make_float2(0.f, 0.f);
-    fft_regs<N, false, true>(v, c.bufB + line * S256::LS, tt, c.tw256);
+    fft_regs<N, false, true>(v, c.bufB() + line * S256::LS, tt, c.tw256());
     // bin kx = tt + 16 r (r < 8) or tt + 16 (r - 16) (r >= 8) goes to reduced-grid column kx mod mx = tt + 16 r'
     float2 w[16];
 #pragma unroll
@@ -425,7 +439,7 @@ __device__ __noinline__ void ph_rows_rhs(const Args& a, const Ctx& c, int slot, 
       const int rp = ((rb % R1) + R1) % R1;
       if (valid && unsigned(cc) < unsigned(L.q_ncol) && __ldg(&qrow[cc]) >= 0) w[rp] = cadd(w[rp], cscale(v[r], scale));
     }
-    fft_x<R1, true, false>(w, c.bufA, c.twx);
+    fft_x<R1, true, false>(w, c.bufA(), c.twx());
     if (M::b_active()) {
       const int rowb = st * 16 + M::b_line(), k1 = M::b_k1();
       if (rowb < L.q_nrow) {
@@ -443,12 +457,12 @@ __device__ __forceinline__ float cg_init(const Args& a, const Ctx& c, int slot, 
   float gsum = 0.f;
   for (int e = threadIdx.x; e < n_unknown; e += TH) {
     const float2 s = __ldcg(&wv[e]);
-    c.ss[e] = s;
-    c.ps[e] = s;
-    c.xs[e] = make_float2(0.f, 0.f);
+    c.ss()[e] = s;
+    c.ps()[e] = s;
+    c.xs()[e] = make_float2(0.f, 0.f);
     gsum += s.x * s.x + s.y * s.y;
   }
-  return block_sum(gsum, c.red);
+  return block_sum(gsum, c.red());
 }
 // Returns true when converged (||C^H r|| <= tol ||C^H d||) or when no progress is possible.
 __device__ __forceinline__ bool cg_update(const Args& a, const Ctx& c, int slot, int n_unknown, float& gamma, float gamma0) {
@@ -461,15 +475,15 @@ __device__ __forceinline__ bool cg_update(const Args& a, const Ctx& c, int slot,
     const int e = threadIdx.x + i * TH;
     if (e < n_unknown) {
       wr[i] = __ldcg(&wv[e]);
-      const float2 p = c.ps[e];
+      const float2 p = c.ps()[e];
       pw += p.x * wr[i].x + p.y * wr[i].y;             // Re(conj(pdir) w) = ||C pdir||^2
     }
   }
   for (int e = threadIdx.x + PER * TH; e < n_unknown; e += TH) {
-    const float2 w = __ldcg(&wv[e]), p = c.ps[e];
+    const float2 w = __ldcg(&wv[e]), p = c.ps()[e];
     pw += p.x * w.x + p.y * w.y;
   }
-  pw = block_sum(pw, c.red);
+  pw = block_sum(pw, c.red());
   if (!(pw > 0.f)) return true;
   const float alpha = gamma / pw;
   float gsum = 0.f;
@@ -477,29 +491,29 @@ __device__ __forceinline__ bool cg_update(const Args& a, const Ctx& c, int slot,
   for (int i = 0; i < PER; ++i) {
     const int e = threadIdx.x + i * TH;
     if (e < n_unknown) {
-      const float2 p = c.ps[e];
-      float2 x = c.xs[e], s = c.ss[e];
+      const float2 p = c.ps()[e];
+      float2 x = c.xs()[e], s = c.ss()[e];
       x.x += alpha * p.x; x.y += alpha * p.y;
       s.x -= alpha * wr[i].x; s.y -= alpha * wr[i].y;
-      c.xs[e] = x;
-      c.ss[e] = s;
+      c.xs()[e] = x;
+      c.ss()[e] = s;
       gsum += s.x * s.x + s.y * s.y;
     }
   }
   for (int e = threadIdx.x + PER * TH; e < n_unknown; e += TH) {
-    const float2 w = __ldcg(&wv[e]), p = c.ps[e];
-    float2 x = c.xs[e], s = c.ss[e];
+    const float2 w = __ldcg(&wv[e]), p = c.ps()[e];
+    float2 x = c.xs()[e], s = c.ss()[e];
     x.x += alpha * p.x; x.y += alpha * p.y;
     s.x -= alpha * w.x; s.y -= alpha * w.y;
-    c.xs[e] = x;
-    c.ss[e] = s;
+    c.xs()[e] = x;
+    c.ss()[e] = s;
     gsum += s.x * s.x + s.y * s.y;
   }
-  gsum = block_sum(gsum, c.red);
+  gsum = block_sum(gsum, c.red());
   const float beta = gsum / gamma;
   for (int e = threadIdx.x; e < n_unknown; e += TH) {
-    const float2 s = c.ss[e], p = c.ps[e];
-    c.ps[e] = make_float2(s.x + beta * p.x, s.y + beta * p.y);
+    const float2 s = c.ss()[e], p = c.ps()[e];
+    c.ps()[e] = make_float2(s.x + beta * p.x, s.y + beta * p.y);
   }
   gamma = gsum;
   return !(gsum > a.tol2 * gamma0);
@@ -508,25 +522,13 @@ __device__ __forceinline__ bool cg_update(const Args& a, const Ctx& c, int slot,
 }  // namespace mg
 
 // ================================================================ the kernel
-__global__ void __launch_bounds__(mg::TH, 2) df_mgrid_kernel(mg::Args a) {
+__global__ void __launch_bounds__(mg::TH, 2) df_mgrid_kernel(const __grid_constant__ mg::Args a) {
   using namespace mg;
-  extern __shared__ float2 dyn[];
-  __shared__ float c_sh[kMaxZern];
-  __shared__ float red[TH / 32];
-  __shared__ DarkDev Lsh;
   Ctx c;
-  c.bufA = dyn;
-  c.bufB = dyn + kXyBuf;
-  float2* tws = dyn + 2 * kXyBuf;                      // [3][256]: rows, columns, N grid
-  c.twx = tws;
-  c.twy = tws + 256;
-  c.tw256 = tws + 512;
-  c.xs = tws + 768;
-  c.ss = c.xs + a.max_unknown;
-  c.ps = c.ss + a.max_unknown;
-  c.c_sh = c_sh;
-  c.red = red;
-  c.L = &Lsh;
+  c.mu = a.max_unknown;
+  float2* tws = c.twx();                               // [3][256]: rows, columns, N grid
+  float* c_sh = c.c_sh();
+  DarkDev& Lsh = *c.Lp();
   const unsigned G = cluster_size(), g = cluster_rank();
   const bool multi = G > 1;
   const int team_id = blockIdx.x / G, n_teams = gridDim.x / G;
@@ -597,7 +599,7 @@ __global__ void __launch_bounds__(mg::TH, 2) df_mgrid_kernel(mg::Args a) {
           const float phi = zern_phase(Lsh.zern + size_t(e) * nz, c_sh, nz);
           float sn, cs;
           sincosf(phi, &sn, &cs);
-          o[Lsh.disc_f[e]] = cmulc(c.xs[e], make_float2(cs, sn));
+          o[Lsh.disc_f[e]] = cmulc(c.xs()[e], make_float2(cs, sn));
         }
         if (g == 0 && threadIdx.x == 0) a.cg_iters[size_t(slot) * a.n_leds + k] = iters;
       }
@@ -611,7 +613,7 @@ void launch_darkfield_mgrid(const DevTables& t, const DarkDev* d_leds, int n_led
                             const float* d_int, int df_iters, float df_tol, int team_size) {
   using namespace mg;
   if (n_leds <= 0) return;
-  const size_t smem = (2 * size_t(kXyBuf) + 768 + 3 * size_t(w.max_unknown)) * sizeof(float2);
+  const size_t smem = (size_t(kSmFixed) + 3 * size_t(w.max_unknown)) * sizeof(float2);
   static bool attr = false;
   static int sms = 148;
   if (!attr) {
