@@ -142,6 +142,9 @@ struct XY {
   static __device__ __forceinline__ int b_k1() { return COLS ? int(threadIdx.x) >> 4 : int(threadIdx.x) % R1; }
   // row layouts in shared memory: X exchange [line][k1][t] with k1-stride 18; Y exchange [line][k'][k1] with k'-stride R1P
   static constexpr int R1P = (R1 == 6) ? 6 : (R1 == 8 || R1 == 10) ? 10 : (R1 == 12) ? 14 : 18;
+  // line stride of the Y exchange: consecutive lines shifted by R1 entries in bank space, so that the
+  // compact layout-B warps (32 / R1 lines each) write conflict-free
+  static constexpr int LSY = 16 * R1P + (R1 % 16);
 };
 
 // Type X: in  v[r] = x[t + 16 r], r < R1 (layout A);  out v[k2] = X[k1 + R1 k2], k2 < 16 (layout B, active threads only).
@@ -192,7 +195,7 @@ __device__ __forceinline__ void fft_y(float2 (&v)[16], float2* __restrict__ buf,
     for (int kp = 0; kp < 16; ++kp) {
       const float2 y = kp ? twmul<INV>(v[kp], tw[k1 * 16 + kp]) : v[0];
       if (COLS) buf[(kp * R1 + k1) * 16 + line] = y;
-      else buf[line * (16 * M::R1P) + kp * M::R1P + k1] = y;
+      else buf[line * M::LSY + kp * M::R1P + k1] = y;
     }
   }
   __syncthreads();
@@ -203,7 +206,7 @@ __device__ __forceinline__ void fft_y(float2 (&v)[16], float2* __restrict__ buf,
 #pragma unroll
       for (int j = 0; j < R1; ++j) a[j] = buf[(kp * R1 + j) * 16 + line];
     } else {
-      const float4* src = reinterpret_cast<const float4*>(buf + line * (16 * M::R1P) + kp * M::R1P);
+      const float4* src = reinterpret_cast<const float4*>(buf + line * M::LSY + kp * M::R1P);
 #pragma unroll
       for (int i = 0; i < R1 / 2; ++i) {
         const float4 q = src[i];
