@@ -114,12 +114,14 @@ struct RegDft<12, INV> {    // 3 x 4: n = 4 n1 + 3 n2, k = 4 k1 + 9 k2
   }
 };
 
-// Host: twiddles of the X/Y exchange, tw[k1 * 16 + t] = e^{-2 pi i t k1 / L}, t < 16, k1 < R1 (L = 16 R1).
-// For R1 = 16 this is the table of fft_core.cuh's N = 256 transform.
+// Host: twiddles of the X/Y exchange, tw[a * 16 + b] = e^{-2 pi i a b / L}, a, b < 16 (L = 16 R1): a symmetric
+// table, read as tw[k1 * 16 + t] by type X and as tw[k' * 16 + k1] by type Y, so that in both the threads of a
+// warp (consecutive t, or consecutive k1) read consecutive entries.  For R1 = 16 this is the table of
+// fft_core.cuh's N = 256 transform.
 inline void build_twiddles_xy(int r1, std::vector<float2>& tw) {
   const int L = 16 * r1;
   tw.assign(256, make_float2(1.f, 0.f));
-  for (int k1 = 0; k1 < r1; ++k1)
+  for (int k1 = 0; k1 < 16; ++k1)
     for (int t = 0; t < 16; ++t) {
       const double a = -2.0 * M_PI * double((t * k1) % L) / double(L);
       tw[k1 * 16 + t] = make_float2(float(std::cos(a)), float(std::sin(a)));
@@ -193,7 +195,7 @@ __device__ __forceinline__ void fft_y(float2 (&v)[16], float2* __restrict__ buf,
     RegDft<16, INV>::run(v);
 #pragma unroll
     for (int kp = 0; kp < 16; ++kp) {
-      const float2 y = kp ? twmul<INV>(v[kp], tw[k1 * 16 + kp]) : v[0];
+      const float2 y = kp ? twmul<INV>(v[kp], tw[kp * 16 + k1]) : v[0];
       if (COLS) buf[(kp * R1 + k1) * 16 + line] = y;
       else buf[line * M::LSY + kp * M::R1P + k1] = y;
     }
