@@ -195,7 +195,7 @@ def main():
     # distinct tiles are generated and repeated to fill the batch, each GPU starting at another tile
     n_gen = min(tiles, 8)
     base = (rank * n_gen) % max(1, cfg.batch - n_gen + 1)
-    stacks, _ = make_batch(cfg, range(base, base + n_gen))
+    stacks, truths = make_batch(cfg, range(base, base + n_gen))
     reps = -(-tiles // n_gen)
     host = np.concatenate([stacks] * reps)[:tiles]
     x = torch.from_numpy(host).cuda()
@@ -308,7 +308,29 @@ def main():
         e2e = {"value": world * k2 * tiles * on * on / 1e6 / dt, "unit": UNIT,
                "h2d_bytes_per_step": int(hx.numel() * 4),
                "d2h_bytes_per_step": int(hf.numel() * 8 + hz.numel() * 4 + hp.numel() * 8 + hs.numel() * 4),
-               "steps": k2, "api": "apic_reconstruct_host (pinned host buffers)"}
+               "steps": k2, "api": "apic_reconstruct_host (pinned host buffers, fp32 intensities)"}
+        if cfg.noise == "poisson":
+            # the same step from the camera's uint16 counts (BASELINE.json config 2: "uint16 raw converted to fp32"):
+            # apic_reconstruct_host_u16, half the host-to-device bytes; reported beside the fp32 number, not instead
+            gains = np.array([[t.gain_bright] * cfg.n_bright + [t.gain_dark] * cfg.n_dark for t in truths])
+            gains = np.concatenate([gains] * reps)[:tiles]
+            raw = np.rint(host.astype(np.float64) * gains[:, :, None, None]).astype(np.uint16)
+            hr = torch.from_numpy(raw).pin_memory()
+            hsc = torch.from_numpy((1.0 / gains).astype(np.float32)).pin_memory()
+            plan.reconstruct_host_u16(hr, hsc, hf, hz, hp, hs, stream)
+            barrier()
+            t0 = time.perf_counter()
+            for _ in range(k2):
+                plan.reconstruct_host_u16(hr, hsc, hf, hz, hp, hs, stream)
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+            if dist:
+                t = torch.tensor([dt], device="cuda")
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                dt = float(t.item())
+            e2e["u16"] = {"value": world * k2 * tiles * on * on / 1e6 / dt, "unit": UNIT,
+                          "h2d_bytes_per_step": int(hr.numel() * 2 + hsc.numel() * 4),
+                          "api": "apic_reconstruct_host_u16 (pinned host buffers, uint16 counts + per-image scale)"}
 
     # ---- the oracle on this box's host cores (rank 0, N = 1 only): one tile of the same workload
     cpu = None

@@ -148,6 +148,24 @@ int apic_reconstruct(apic_plan* plan, const float* d_intensity, int batch, float
 int apic_reconstruct_host(apic_plan* plan, const float* h_intensity, int batch, float* h_field,
                           float* h_zernike, float* h_pupil, int32_t* h_status, void* cuda_stream);
 
+/* The same reconstruction from raw camera counts (BASELINE.json config 2: "uint16 raw converted to
+ * fp32"; exposures differ between NA-matching and darkfield frames,
+ * PAPER.md:199):
+ *   d_raw    [batch][n_bright+n_dark][N][N] uint16, same order as d_intensity
+ *   d_scale  [batch][n_bright+n_dark] float: intensity = count * scale (1 / (gain * exposure) of
+ *            that frame, so that all frames are in common radiometric units, R17)
+ * The conversion is fused into the S0 statistics pass (one read of the counts, one fp32 working
+ * copy owned by the plan, allocated on first use: max_batch * n_img * N * N * 4 bytes); every later
+ * step is the fp32 path, so the results equal apic_reconstruct on float(count) * scale bit for bit.
+ * A non-finite scale makes the tile APIC_TILE_BAD_INPUT.  Other arguments as apic_reconstruct. */
+int apic_reconstruct_u16(apic_plan* plan, const uint16_t* d_raw, const float* d_scale, int batch,
+                         float* d_field, float* d_zernike, float* d_pupil, int32_t* d_status,
+                         void* cuda_stream);
+/* ... and with HOST buffers (half the host-to-device bytes of apic_reconstruct_host). */
+int apic_reconstruct_host_u16(apic_plan* plan, const uint16_t* h_raw, const float* h_scale, int batch,
+                              float* h_field, float* h_zernike, float* h_pupil, int32_t* h_status,
+                              void* cuda_stream);
+
 /* Stage-level access for parity tests (device pointers, valid after apic_reconstruct on the
  * same stream, for the tiles of the LAST internal chunk; tile index is chunk-local):
  *   APIC_DBG_SUBSPECTRA: [chunk][sum_i |D_i|] complex64, S_hat_i on D_i (Eq. 7), LED-major, bins

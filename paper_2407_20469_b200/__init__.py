@@ -21,7 +21,7 @@ TILE_OK, TILE_BACKGROUND, TILE_BAD_INPUT, TILE_SOLVE_FAILED = 0, 1, 2, 3
 DBG_SUBSPECTRA, DBG_OBJECT_SPECTRUM, DBG_DF_ITERS = 0, 1, 2
 
 EXPORTS = ("apic_params_default", "apic_plan_create", "apic_plan_destroy", "apic_plan_info",
-           "apic_geometry_info", "apic_geometry_dark_grids", "apic_plan_dark_sets", "apic_reconstruct", "apic_reconstruct_host",
+           "apic_geometry_info", "apic_geometry_dark_grids", "apic_plan_dark_sets", "apic_reconstruct", "apic_reconstruct_host", "apic_reconstruct_u16", "apic_reconstruct_host_u16",
            "apic_debug_buffer", "apic_debug_copy", "apic_fft2d", "apic_fft2d_xy", "apic_last_launch_count", "apic_strerror",
            "apic_last_cuda_error", "apic_version", "apic_profile_categories", "apic_profile_category_name",
            "apic_profile_begin", "apic_profile_end", "apic_profile_work")
@@ -76,6 +76,9 @@ def load() -> C.CDLL:
     lib.apic_reconstruct.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
                                      C.c_void_p, C.c_void_p]
     lib.apic_reconstruct_host.argtypes = lib.apic_reconstruct.argtypes
+    lib.apic_reconstruct_u16.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
+                                         C.c_void_p, C.c_void_p]
+    lib.apic_reconstruct_host_u16.argtypes = lib.apic_reconstruct_u16.argtypes
     lib.apic_debug_buffer.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)]
     lib.apic_debug_copy.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p]
     lib.apic_fft2d.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
@@ -210,6 +213,42 @@ class Plan:
                                           pupil.data_ptr() if pupil is not None else None, status.data_ptr(),
                                           C.c_void_p(stream)), "apic_reconstruct")
         return field, zern, pupil, status
+
+    def reconstruct_u16(self, raw, scale, want_pupil: bool = True, out=None):
+        """raw: uint16 CUDA tensor [B][n_img][N][N] (camera counts), scale: float32 CUDA tensor [B][n_img]
+        (intensity = count * scale).  Returns the same tuple as ``reconstruct``."""
+        import torch
+        if not (raw.is_cuda and raw.dtype == torch.uint16 and raw.is_contiguous()):
+            raise ApicError("raw must be a contiguous uint16 CUDA tensor")
+        b = raw.shape[0]
+        if tuple(raw.shape[1:]) != (self.n_img, self.n, self.n):
+            raise ApicError(f"raw shape {tuple(raw.shape)} != [B,{self.n_img},{self.n},{self.n}]")
+        if not (scale.is_cuda and scale.dtype == torch.float32 and scale.is_contiguous()
+                and tuple(scale.shape) == (b, self.n_img)):
+            raise ApicError(f"scale must be a contiguous float32 CUDA tensor [{b},{self.n_img}]")
+        dev = raw.device
+        if out is None:
+            field = torch.empty((b, self.out_n, self.out_n), dtype=torch.complex64, device=dev)
+            zern = torch.empty((b, self.nz), dtype=torch.float32, device=dev)
+            pupil = torch.empty((b, self.n, self.n), dtype=torch.complex64, device=dev) if want_pupil else None
+            status = torch.empty((b,), dtype=torch.int32, device=dev)
+        else:
+            field, zern, pupil, status = out
+        stream = torch.cuda.current_stream(dev).cuda_stream
+        _check(self._lib.apic_reconstruct_u16(self._h, raw.data_ptr(), scale.data_ptr(), b, field.data_ptr(),
+                                              zern.data_ptr(), pupil.data_ptr() if pupil is not None else None,
+                                              status.data_ptr(), C.c_void_p(stream)), "apic_reconstruct_u16")
+        return field, zern, pupil, status
+
+    def reconstruct_host_u16(self, raw, scale, field, zern, pupil, status, stream: int = 0):
+        """Host buffers (numpy arrays or CPU torch tensors, ideally pinned); blocking."""
+        def ptr(a):
+            if a is None:
+                return None
+            return a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr()
+        b = raw.shape[0]
+        _check(self._lib.apic_reconstruct_host_u16(self._h, ptr(raw), ptr(scale), b, ptr(field), ptr(zern), ptr(pupil),
+                                                   ptr(status), C.c_void_p(stream)), "apic_reconstruct_host_u16")
 
     def reconstruct_host(self, intensity, field, zern, pupil, status, stream: int = 0):
         """Host buffers (numpy arrays or CPU torch tensors, ideally pinned); blocking."""

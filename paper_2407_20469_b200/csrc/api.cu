@@ -44,6 +44,10 @@ struct apic_plan {
   int32_t* st_status = nullptr;
   int st_batch = 0;
   bool st_has_pupil = false;
+  float* cv_int = nullptr;           // fp32 copy of a uint16 batch (apic_reconstruct_u16), allocated on first use
+  uint16_t* st_raw = nullptr;        // staging of apic_reconstruct_host_u16
+  float* st_scale = nullptr;
+  int st_raw_batch = 0, st_int_batch = 0;
 
   template <class T>
   bool dalloc(T** p, size_t count, bool table) {
@@ -149,6 +153,7 @@ int apic_plan_destroy(apic_plan* plan) {
   if (plan->h_live_count) cudaFreeHost(plan->h_live_count);
   cudaFree(plan->st_int); cudaFree(plan->st_field); cudaFree(plan->st_zern); cudaFree(plan->st_pupil);
   cudaFree(plan->st_status);
+  cudaFree(plan->cv_int); cudaFree(plan->st_raw); cudaFree(plan->st_scale);
   delete plan;
   return APIC_OK;
 }
@@ -312,11 +317,18 @@ int apic_plan_dark_sets(const apic_plan* plan, int* led, int* n_unknown, int* n_
   return APIC_OK;
 }
 
-int apic_reconstruct(apic_plan* plan, const float* d_intensity, int batch, float* d_field, float* d_zernike,
-                     float* d_pupil, int32_t* d_status, void* cuda_stream) {
-  if (!plan || !d_intensity || !d_field || !d_zernike || !d_status) return APIC_EINVAL;
+// The whole path.  Either d_intensity (fp32) or d_raw + d_scale (uint16 counts and the per-image factor that
+// turns them into radiometric units) is given; the uint16 form is converted inside the S0 statistics pass.
+static int reconstruct_impl(apic_plan* plan, const float* d_intensity, const uint16_t* d_raw, const float* d_scale, int batch,
+                            float* d_field, float* d_zernike, float* d_pupil, int32_t* d_status, void* cuda_stream) {
+  if (!plan || !(d_intensity || (d_raw && d_scale)) || !d_field || !d_zernike || !d_status) return APIC_EINVAL;
   if (batch < 1 || batch > plan->params.max_batch) return APIC_EBATCH;
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  if (d_raw && !plan->cv_int) {
+    const size_t bytes = size_t(plan->params.max_batch) * plan->dev.n_img * plan->dev.n * plan->dev.n * sizeof(float);
+    if (!cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->cv_int), bytes), "cudaMalloc uint16 conversion buffer")) return APIC_ENOMEM;
+    plan->workspace_bytes += bytes;
+  }
   const DevTables& t = plan->dev;
   const Workspace& w = plan->ws;
   const apic_params& p = plan->params;
@@ -325,7 +337,12 @@ int apic_reconstruct(apic_plan* plan, const float* d_intensity, int batch, float
   // S0: statistics, status, list of tiles to reconstruct
   {
     LaunchCtx c{s, &plan->launches, &plan->prof, plan->bs.live, plan->bs.live_count, 0, batch};
-    launch_image_stats(t, d_intensity, batch, plan->bs.stats, c);
+    if (d_raw) {
+      launch_image_stats_u16(t, d_raw, d_scale, plan->cv_int, batch, plan->bs.stats, c);
+      d_intensity = plan->cv_int;
+    } else {
+      launch_image_stats(t, d_intensity, batch, plan->bs.stats, c);
+    }
     launch_tile_status(t, plan->bs.stats, batch, p.bg_mode, p.bg_threshold, d_status, plan->bs.live,
                        plan->bs.live_count, c);
     launch_zero_dead(t, d_status, batch, d_field, d_zernike, d_pupil, c);
@@ -361,23 +378,52 @@ int apic_reconstruct(apic_plan* plan, const float* d_intensity, int batch, float
   return APIC_OK;
 }
 
+int apic_reconstruct(apic_plan* plan, const float* d_intensity, int batch, float* d_field, float* d_zernike,
+                     float* d_pupil, int32_t* d_status, void* cuda_stream) {
+  if (!d_intensity) return APIC_EINVAL;
+  return reconstruct_impl(plan, d_intensity, nullptr, nullptr, batch, d_field, d_zernike, d_pupil, d_status, cuda_stream);
+}
+
+int apic_reconstruct_u16(apic_plan* plan, const uint16_t* d_raw, const float* d_scale, int batch, float* d_field,
+                         float* d_zernike, float* d_pupil, int32_t* d_status, void* cuda_stream) {
+  if (!d_raw || !d_scale) return APIC_EINVAL;
+  return reconstruct_impl(plan, nullptr, d_raw, d_scale, batch, d_field, d_zernike, d_pupil, d_status, cuda_stream);
+}
+
+// Host-buffer form of both entries: H2D, reconstruct, D2H, one synchronisation.
+static int reconstruct_host_impl(apic_plan* plan, const float* h_intensity, const uint16_t* h_raw, const float* h_scale,
+                                 int batch, float* h_field, float* h_zernike, float* h_pupil, int32_t* h_status,
+                                 void* cuda_stream);
+
 int apic_reconstruct_host(apic_plan* plan, const float* h_intensity, int batch, float* h_field, float* h_zernike,
                           float* h_pupil, int32_t* h_status, void* cuda_stream) {
-  if (!plan || !h_intensity || !h_field || !h_zernike || !h_status) return APIC_EINVAL;
+  if (!h_intensity) return APIC_EINVAL;
+  return reconstruct_host_impl(plan, h_intensity, nullptr, nullptr, batch, h_field, h_zernike, h_pupil, h_status, cuda_stream);
+}
+
+int apic_reconstruct_host_u16(apic_plan* plan, const uint16_t* h_raw, const float* h_scale, int batch, float* h_field,
+                              float* h_zernike, float* h_pupil, int32_t* h_status, void* cuda_stream) {
+  if (!h_raw || !h_scale) return APIC_EINVAL;
+  return reconstruct_host_impl(plan, nullptr, h_raw, h_scale, batch, h_field, h_zernike, h_pupil, h_status, cuda_stream);
+}
+
+static int reconstruct_host_impl(apic_plan* plan, const float* h_intensity, const uint16_t* h_raw, const float* h_scale,
+                                 int batch, float* h_field, float* h_zernike, float* h_pupil, int32_t* h_status,
+                                 void* cuda_stream) {
+  if (!plan || !h_field || !h_zernike || !h_status) return APIC_EINVAL;
   if (batch < 1 || batch > plan->params.max_batch) return APIC_EBATCH;
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   const DevTables& t = plan->dev;
   const size_t nn = size_t(t.n) * t.n, on = size_t(t.n) * t.u;
-  const size_t b_int = size_t(batch) * t.n_img * nn * sizeof(float), b_field = size_t(batch) * on * on * 2 * sizeof(float);
+  const size_t n_px = size_t(batch) * t.n_img * nn;
+  const size_t b_field = size_t(batch) * on * on * 2 * sizeof(float);
   const size_t b_zern = size_t(batch) * t.nz * sizeof(float), b_pupil = size_t(batch) * nn * 2 * sizeof(float);
   if (batch > plan->st_batch || (h_pupil && !plan->st_has_pupil)) {
-    cudaFree(plan->st_int); cudaFree(plan->st_field); cudaFree(plan->st_zern); cudaFree(plan->st_pupil);
-    cudaFree(plan->st_status);
-    plan->st_int = plan->st_field = plan->st_zern = plan->st_pupil = nullptr;
+    cudaFree(plan->st_field); cudaFree(plan->st_zern); cudaFree(plan->st_pupil); cudaFree(plan->st_status);
+    plan->st_field = plan->st_zern = plan->st_pupil = nullptr;
     plan->st_status = nullptr;
     plan->st_batch = 0;
-    bool ok = cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->st_int), b_int), "cudaMalloc staging") &&
-              cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->st_field), b_field), "cudaMalloc staging") &&
+    bool ok = cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->st_field), b_field), "cudaMalloc staging") &&
               cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->st_zern), b_zern), "cudaMalloc staging") &&
               cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->st_status), size_t(batch) * sizeof(int32_t)), "cudaMalloc staging");
     if (ok && h_pupil) ok = cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->st_pupil), b_pupil), "cudaMalloc staging");
@@ -385,9 +431,32 @@ int apic_reconstruct_host(apic_plan* plan, const float* h_intensity, int batch, 
     plan->st_batch = batch;
     plan->st_has_pupil = h_pupil != nullptr;
   }
-  if (!cuda_ok(cudaMemcpyAsync(plan->st_int, h_intensity, b_int, cudaMemcpyHostToDevice, s), "H2D")) return APIC_ECUDA;
-  const int rc = apic_reconstruct(plan, plan->st_int, batch, plan->st_field, plan->st_zern,
-                                  h_pupil ? plan->st_pupil : nullptr, plan->st_status, s);
+  int rc;
+  if (h_raw) {
+    if (batch > plan->st_raw_batch) {
+      cudaFree(plan->st_raw); cudaFree(plan->st_scale);
+      plan->st_raw = nullptr; plan->st_scale = nullptr; plan->st_raw_batch = 0;
+      if (!cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->st_raw), n_px * sizeof(uint16_t)), "cudaMalloc staging") ||
+          !cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->st_scale), size_t(batch) * t.n_img * sizeof(float)), "cudaMalloc staging"))
+        return APIC_ENOMEM;
+      plan->st_raw_batch = batch;
+    }
+    if (!cuda_ok(cudaMemcpyAsync(plan->st_raw, h_raw, n_px * sizeof(uint16_t), cudaMemcpyHostToDevice, s), "H2D")) return APIC_ECUDA;
+    if (!cuda_ok(cudaMemcpyAsync(plan->st_scale, h_scale, size_t(batch) * t.n_img * sizeof(float), cudaMemcpyHostToDevice, s), "H2D"))
+      return APIC_ECUDA;
+    rc = apic_reconstruct_u16(plan, plan->st_raw, plan->st_scale, batch, plan->st_field, plan->st_zern,
+                              h_pupil ? plan->st_pupil : nullptr, plan->st_status, s);
+  } else {
+    if (batch > plan->st_int_batch) {
+      cudaFree(plan->st_int);
+      plan->st_int = nullptr; plan->st_int_batch = 0;
+      if (!cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->st_int), n_px * sizeof(float)), "cudaMalloc staging")) return APIC_ENOMEM;
+      plan->st_int_batch = batch;
+    }
+    if (!cuda_ok(cudaMemcpyAsync(plan->st_int, h_intensity, n_px * sizeof(float), cudaMemcpyHostToDevice, s), "H2D")) return APIC_ECUDA;
+    rc = apic_reconstruct(plan, plan->st_int, batch, plan->st_field, plan->st_zern, h_pupil ? plan->st_pupil : nullptr,
+                          plan->st_status, s);
+  }
   if (rc != APIC_OK) return rc;
   cudaMemcpyAsync(h_field, plan->st_field, b_field, cudaMemcpyDeviceToHost, s);
   cudaMemcpyAsync(h_zernike, plan->st_zern, b_zern, cudaMemcpyDeviceToHost, s);

@@ -49,6 +49,52 @@ void launch_image_stats(const DevTables& t, const float* d_int, int batch, doubl
   image_stats_kernel<<<grid, 256, 0, c.stream>>>(d_int, t.n * t.n, t.n_img, stats);
 }
 
+// uint16 entry (apic_reconstruct_u16): the statistics pass also converts count * scale into the fp32 working copy
+__global__ void __launch_bounds__(256) image_stats_u16_kernel(const uint16_t* __restrict__ d_raw, const float* __restrict__ d_scale,
+                                                              float* __restrict__ d_out, int npix, int n_img,
+                                                              double* __restrict__ stats) {
+  const int img = blockIdx.x, tile = blockIdx.y;
+  const size_t off = (size_t(tile) * n_img + img) * npix;
+  const uint4* p = reinterpret_cast<const uint4*>(d_raw + off);          // 8 pixels
+  float4* o = reinterpret_cast<float4*>(d_out + off);
+  const float sc = d_scale[size_t(tile) * n_img + img];
+  float s = 0.f, q = 0.f;
+  for (int i = threadIdx.x; i < npix / 8; i += 256) {
+    const uint4 r = __ldg(&p[i]);
+    float4 a, b;
+    a.x = float(r.x & 0xffffu) * sc; a.y = float(r.x >> 16) * sc; a.z = float(r.y & 0xffffu) * sc; a.w = float(r.y >> 16) * sc;
+    b.x = float(r.z & 0xffffu) * sc; b.y = float(r.z >> 16) * sc; b.z = float(r.w & 0xffffu) * sc; b.w = float(r.w >> 16) * sc;
+    o[2 * i] = a;
+    o[2 * i + 1] = b;
+    // same association as image_stats_kernel, so that the statistics equal those of the fp32 entry on the same values
+    s += (a.x + a.y) + (a.z + a.w);
+    q += (a.x * a.x + a.y * a.y) + (a.z * a.z + a.w * a.w);
+    s += (b.x + b.y) + (b.z + b.w);
+    q += (b.x * b.x + b.y * b.y) + (b.z * b.z + b.w * b.w);
+  }
+  __shared__ double sh[3][256];
+  sh[0][threadIdx.x] = s;
+  sh[1][threadIdx.x] = q;
+  sh[2][threadIdx.x] = isfinite(sc) ? 0.0 : double(threadIdx.x == 0);      // counts are finite; a non-finite scale is bad input
+  __syncthreads();
+  for (int o2 = 128; o2 > 0; o2 >>= 1) {
+    if (threadIdx.x < o2) {
+      sh[0][threadIdx.x] += sh[0][threadIdx.x + o2];
+      sh[1][threadIdx.x] += sh[1][threadIdx.x + o2];
+      sh[2][threadIdx.x] += sh[2][threadIdx.x + o2];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x < 3) stats[(size_t(tile) * n_img + img) * 3 + threadIdx.x] = sh[threadIdx.x][0];
+}
+
+void launch_image_stats_u16(const DevTables& t, const uint16_t* d_raw, const float* d_scale, float* d_out, int batch,
+                            double* stats, const LaunchCtx& c) {
+  dim3 grid(t.n_img, batch);
+  ProfScope ps(c, CAT_STATS);
+  image_stats_u16_kernel<<<grid, 256, 0, c.stream>>>(d_raw, d_scale, d_out, t.n * t.n, t.n_img, stats);
+}
+
 // one warp: per-tile status (O1, BASELINE.json item 5, R18) and the ordered list of
 // tiles to reconstruct
 __global__ void tile_status_kernel(const double* __restrict__ stats, int batch, int n_img, int nb, int npix,

@@ -144,6 +144,9 @@ struct ProfScope {
 };
 
 void launch_image_stats(const DevTables& t, const float* d_int, int batch, double* stats, const LaunchCtx& c);
+// the same pass over uint16 counts: converts (count * scale[tile][image]) into d_out (fp32, same layout) on the way
+void launch_image_stats_u16(const DevTables& t, const uint16_t* d_raw, const float* d_scale, float* d_out, int batch,
+                            double* stats, const LaunchCtx& c);
 void launch_tile_status(const DevTables& t, const double* stats, int batch, int bg_mode, float bg_thr,
                         int32_t* status, int32_t* live, int32_t* live_count, const LaunchCtx& c);
 void launch_zero_dead(const DevTables& t, const int32_t* status, int batch, float* field, float* zern,

@@ -267,3 +267,36 @@ def test_host_entry_point_and_batch_limits(A):
     with pytest.raises(A.ApicError, match="batch"):
         plan.reconstruct(big)
     assert plan.last_launch_count > 0
+
+
+def test_uint16_entry_equals_fp32_entry_on_the_same_values(A):
+    """apic_reconstruct_u16 (raw counts + per-image scale, conversion fused into the S0 pass) must give
+    the fp32 entry's bits on float(count) * scale, through the device and the host entry points; a
+    non-finite scale is bad input."""
+    import torch
+    cfg = get_config(2, tile_n=64, batch=4, grid=(2, 2))
+    stacks, truths = make_batch(cfg, [0, 1, 2, 3])
+    nb = cfg.n_bright
+    gains = np.array([[t.gain_bright] * nb + [t.gain_dark] * cfg.n_dark for t in truths])        # photons per unit
+    raw = np.rint(stacks.astype(np.float64) * gains[:, :, None, None])
+    assert raw.min() >= 0 and raw.max() <= 65535
+    raw = raw.astype(np.uint16)
+    scale = (1.0 / gains).astype(np.float32)
+    x32 = raw.astype(np.float32) * scale[:, :, None, None]                                          # fp32 product
+    assert np.allclose(x32, stacks, rtol=1e-6)
+    plan = A.Plan.from_config(cfg, max_batch=4)
+    ref = [o.cpu().numpy() for o in plan.reconstruct(torch.from_numpy(x32).cuda())]
+    got = [o.cpu().numpy() for o in plan.reconstruct_u16(torch.from_numpy(raw).cuda(), torch.from_numpy(scale).cuda())]
+    for a, b in zip(ref, got):
+        assert np.array_equal(a, b)
+    assert np.all(ref[3] == 0)
+    # host entry
+    field = np.empty_like(ref[0]); zern = np.empty_like(ref[1]); pupil = np.empty_like(ref[2]); status = np.empty_like(ref[3])
+    plan.reconstruct_host_u16(raw, scale, field, zern, pupil, status)
+    assert np.array_equal(field, ref[0]) and np.array_equal(zern, ref[1]) and np.array_equal(status, ref[3])
+    # a non-finite scale flags the tile and leaves the others untouched
+    bad = scale.copy()
+    bad[2, 5] = np.inf
+    got = [o.cpu().numpy() for o in plan.reconstruct_u16(torch.from_numpy(raw).cuda(), torch.from_numpy(bad).cuda())]
+    assert list(got[3]) == [0, 0, 2, 0] and np.all(got[0][2] == 0)
+    assert np.array_equal(got[0][[0, 1, 3]], ref[0][[0, 1, 3]])
