@@ -81,7 +81,7 @@ typedef struct {
                             kernel (one launch per LED and pass), 3 = team kernel on the full
                             N x N grid.  At N = 256 mode 0 runs the CG mat-vecs on per-LED
                             reduced cyclic grids; other N: same as 3     */
-  int df_team;           /* df_mode 0: CTAs (= SMs) per tile, 1 | 2 | 4 | 8; 0 = chosen from the
+  int df_team;           /* df_mode 0 / 3: CTAs per tile, 1 | 2 | 4 | 8; 0 = chosen from the
                             pass size (as many as the pass leaves SMs for)                      */
 } apic_params;
 

@@ -48,6 +48,10 @@ struct apic_plan {
   uint16_t* st_raw = nullptr;        // staging of apic_reconstruct_host_u16
   float* st_scale = nullptr;
   int st_raw_batch = 0, st_int_batch = 0;
+  // apic_reconstruct_host: copy streams and per-part events (upload done, kernels done) + one for the caller's stream
+  static constexpr int kMaxParts = 4;
+  cudaStream_t copy_in = nullptr, copy_out = nullptr;
+  cudaEvent_t part_ev[2 * kMaxParts + 1] = {};
 
   template <class T>
   bool dalloc(T** p, size_t count, bool table) {
@@ -154,6 +158,10 @@ int apic_plan_destroy(apic_plan* plan) {
   cudaFree(plan->st_int); cudaFree(plan->st_field); cudaFree(plan->st_zern); cudaFree(plan->st_pupil);
   cudaFree(plan->st_status);
   cudaFree(plan->cv_int); cudaFree(plan->st_raw); cudaFree(plan->st_scale);
+  if (plan->copy_in) {
+    cudaStreamDestroy(plan->copy_in); cudaStreamDestroy(plan->copy_out);
+    for (cudaEvent_t e : plan->part_ev) if (e) cudaEventDestroy(e);
+  }
   delete plan;
   return APIC_OK;
 }
@@ -431,7 +439,6 @@ static int reconstruct_host_impl(apic_plan* plan, const float* h_intensity, cons
     plan->st_batch = batch;
     plan->st_has_pupil = h_pupil != nullptr;
   }
-  int rc;
   if (h_raw) {
     if (batch > plan->st_raw_batch) {
       cudaFree(plan->st_raw); cudaFree(plan->st_scale);
@@ -441,27 +448,62 @@ static int reconstruct_host_impl(apic_plan* plan, const float* h_intensity, cons
         return APIC_ENOMEM;
       plan->st_raw_batch = batch;
     }
-    if (!cuda_ok(cudaMemcpyAsync(plan->st_raw, h_raw, n_px * sizeof(uint16_t), cudaMemcpyHostToDevice, s), "H2D")) return APIC_ECUDA;
-    if (!cuda_ok(cudaMemcpyAsync(plan->st_scale, h_scale, size_t(batch) * t.n_img * sizeof(float), cudaMemcpyHostToDevice, s), "H2D"))
-      return APIC_ECUDA;
-    rc = apic_reconstruct_u16(plan, plan->st_raw, plan->st_scale, batch, plan->st_field, plan->st_zern,
-                              h_pupil ? plan->st_pupil : nullptr, plan->st_status, s);
-  } else {
-    if (batch > plan->st_int_batch) {
-      cudaFree(plan->st_int);
-      plan->st_int = nullptr; plan->st_int_batch = 0;
-      if (!cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->st_int), n_px * sizeof(float)), "cudaMalloc staging")) return APIC_ENOMEM;
-      plan->st_int_batch = batch;
-    }
-    if (!cuda_ok(cudaMemcpyAsync(plan->st_int, h_intensity, n_px * sizeof(float), cudaMemcpyHostToDevice, s), "H2D")) return APIC_ECUDA;
-    rc = apic_reconstruct(plan, plan->st_int, batch, plan->st_field, plan->st_zern, h_pupil ? plan->st_pupil : nullptr,
-                          plan->st_status, s);
+  } else if (batch > plan->st_int_batch) {
+    cudaFree(plan->st_int);
+    plan->st_int = nullptr; plan->st_int_batch = 0;
+    if (!cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->st_int), n_px * sizeof(float)), "cudaMalloc staging")) return APIC_ENOMEM;
+    plan->st_int_batch = batch;
   }
-  if (rc != APIC_OK) return rc;
-  cudaMemcpyAsync(h_field, plan->st_field, b_field, cudaMemcpyDeviceToHost, s);
-  cudaMemcpyAsync(h_zernike, plan->st_zern, b_zern, cudaMemcpyDeviceToHost, s);
-  if (h_pupil) cudaMemcpyAsync(h_pupil, plan->st_pupil, b_pupil, cudaMemcpyDeviceToHost, s);
-  cudaMemcpyAsync(h_status, plan->st_status, size_t(batch) * sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+  if (!plan->copy_in) {
+    bool ok = cuda_ok(cudaStreamCreateWithFlags(&plan->copy_in, cudaStreamNonBlocking), "cudaStreamCreate") &&
+              cuda_ok(cudaStreamCreateWithFlags(&plan->copy_out, cudaStreamNonBlocking), "cudaStreamCreate");
+    for (int k = 0; ok && k < 2 * apic_plan::kMaxParts + 1; ++k)
+      ok = cuda_ok(cudaEventCreateWithFlags(&plan->part_ev[k], cudaEventDisableTiming), "cudaEventCreate");
+    if (!ok) return APIC_ECUDA;
+  }
+  // Sub-batches of >= 32 tiles (a smaller pass leaves the darkfield teams too few tiles to fill the GPU): the
+  // upload of part i+1 and the download of part i-1 run on their own streams beside the kernels of part i.
+  // Results do not depend on the split (a tile's result is independent of its batch; tested).
+  const int parts = std::max(1, std::min(apic_plan::kMaxParts, batch / 32));
+  const int per = (batch + parts - 1) / parts;
+  const size_t img_px = size_t(t.n_img) * nn;
+  cudaEventRecord(plan->part_ev[2 * apic_plan::kMaxParts], s);                 // earlier work on the caller's stream
+  cudaStreamWaitEvent(plan->copy_in, plan->part_ev[2 * apic_plan::kMaxParts], 0);
+  cudaStreamWaitEvent(plan->copy_out, plan->part_ev[2 * apic_plan::kMaxParts], 0);
+  for (int k = 0, b0 = 0; b0 < batch; ++k, b0 += per) {
+    const int nb = std::min(per, batch - b0);
+    if (h_raw) {
+      cudaMemcpyAsync(plan->st_raw + b0 * img_px, h_raw + b0 * img_px, nb * img_px * sizeof(uint16_t), cudaMemcpyHostToDevice,
+                      plan->copy_in);
+      cudaMemcpyAsync(plan->st_scale + size_t(b0) * t.n_img, h_scale + size_t(b0) * t.n_img, size_t(nb) * t.n_img * sizeof(float),
+                      cudaMemcpyHostToDevice, plan->copy_in);
+    } else {
+      cudaMemcpyAsync(plan->st_int + b0 * img_px, h_intensity + b0 * img_px, nb * img_px * sizeof(float), cudaMemcpyHostToDevice,
+                      plan->copy_in);
+    }
+    cudaEventRecord(plan->part_ev[2 * k], plan->copy_in);
+  }
+  for (int k = 0, b0 = 0; b0 < batch; ++k, b0 += per) {
+    const int nb = std::min(per, batch - b0);
+    cudaStreamWaitEvent(s, plan->part_ev[2 * k], 0);
+    float* f = plan->st_field + size_t(b0) * on * on * 2;
+    float* z = plan->st_zern + size_t(b0) * t.nz;
+    float* pu = h_pupil ? plan->st_pupil + size_t(b0) * nn * 2 : nullptr;
+    int32_t* st = plan->st_status + b0;
+    const int rc = h_raw ? apic_reconstruct_u16(plan, plan->st_raw + b0 * img_px, plan->st_scale + size_t(b0) * t.n_img, nb, f, z, pu, st, s)
+                         : apic_reconstruct(plan, plan->st_int + b0 * img_px, nb, f, z, pu, st, s);
+    if (rc != APIC_OK) {
+      cudaStreamSynchronize(plan->copy_in); cudaStreamSynchronize(plan->copy_out); cudaStreamSynchronize(s);
+      return rc;
+    }
+    cudaEventRecord(plan->part_ev[2 * k + 1], s);
+    cudaStreamWaitEvent(plan->copy_out, plan->part_ev[2 * k + 1], 0);
+    cudaMemcpyAsync(h_field + size_t(b0) * on * on * 2, f, size_t(nb) * on * on * 2 * sizeof(float), cudaMemcpyDeviceToHost, plan->copy_out);
+    cudaMemcpyAsync(h_zernike + size_t(b0) * t.nz, z, size_t(nb) * t.nz * sizeof(float), cudaMemcpyDeviceToHost, plan->copy_out);
+    if (h_pupil) cudaMemcpyAsync(h_pupil + size_t(b0) * nn * 2, pu, size_t(nb) * nn * 2 * sizeof(float), cudaMemcpyDeviceToHost, plan->copy_out);
+    cudaMemcpyAsync(h_status + b0, st, size_t(nb) * sizeof(int32_t), cudaMemcpyDeviceToHost, plan->copy_out);
+  }
+  if (!cuda_ok(cudaStreamSynchronize(plan->copy_out), "apic_reconstruct_host")) return APIC_ECUDA;
   if (!cuda_ok(cudaStreamSynchronize(s), "apic_reconstruct_host")) return APIC_ECUDA;
   return APIC_OK;
 }

@@ -634,8 +634,12 @@ void launch_darkfield_mgrid(const DevTables& t, const DarkDev* d_leds, int n_led
     int per_sm = 1;
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, df_mgrid_kernel, TH, smem);
     per_sm = std::max(1, per_sm);
+    // as many CTAs per tile as the pass leaves resident slots for.  Measured on config 2 (ms per step): 32 tiles
+    // G = 8: 8.3; 56 tiles G = 5: 10.4; 64 tiles G = 4: 12.1; cluster sizes 6 and 7 place badly (40 tiles G = 7: 15.7,
+    // 48 tiles G = 6: 16.3) and are skipped.
     G = 1;
-    while (G < 8 && 2 * G * c.chunk_tiles <= sms * per_sm) G *= 2;
+    for (int cand : {8, 5, 4, 2})
+      if (cand * c.chunk_tiles <= sms * per_sm) { G = cand; break; }
   }
   cudaLaunchConfig_t cfg{};
   cudaLaunchAttribute at[1];

@@ -300,3 +300,21 @@ def test_uint16_entry_equals_fp32_entry_on_the_same_values(A):
     got = [o.cpu().numpy() for o in plan.reconstruct_u16(torch.from_numpy(raw).cuda(), torch.from_numpy(bad).cuda())]
     assert list(got[3]) == [0, 0, 2, 0] and np.all(got[0][2] == 0)
     assert np.array_equal(got[0][[0, 1, 3]], ref[0][[0, 1, 3]])
+
+
+def test_host_entry_pipelines_sub_batches_without_changing_bits(A):
+    """apic_reconstruct_host splits batches of >= 64 tiles into sub-batches whose uploads / kernels /
+    downloads overlap on separate streams: same bits as one device call on the whole batch."""
+    import torch
+    cfg = get_config(2, tile_n=64, batch=4, grid=(2, 2))
+    stacks, _ = make_batch(cfg, [0, 1, 2, 3])
+    big = np.ascontiguousarray(np.concatenate([stacks] * 18)[:70])
+    plan = A.Plan.from_config(cfg, max_batch=70)
+    ref = [o.cpu().numpy() for o in plan.reconstruct(torch.from_numpy(big).cuda())]
+    field = np.empty_like(ref[0]); zern = np.empty_like(ref[1]); pupil = np.empty_like(ref[2]); status = np.empty_like(ref[3])
+    for _ in range(2):
+        field[:] = 0
+        plan.reconstruct_host(big, field, zern, pupil, status)
+        assert np.array_equal(field, ref[0]) and np.array_equal(zern, ref[1])
+        assert np.array_equal(pupil, ref[2]) and np.array_equal(status, ref[3])
+    assert np.array_equal(field[0], field[4]) and np.array_equal(field[1], field[69])
