@@ -269,8 +269,21 @@ def main():
         flop_per_launch, note = None, "no flop model for this kernel"
     achieved = flop_per_launch / (avg_ms * 1e-3) / 1e12 if (samples and flop_per_launch) else None
     share = (avg_ms * nlaunch / total_kernel_ms) if total_kernel_ms else None
+    # DRAM bytes per launch of that kernel from the committed ncu --set full capture (same workload only)
+    traffic = None
+    if dominant == "df_persistent" and args.config == 2 and tiles == 64 and args.df_mode == 0:
+        try:
+            import csv
+            with open(os.path.join(ROOT, "profiles", "r1b_traffic_cfg2.csv")) as fh:
+                row = next(r for r in csv.DictReader(fh) if r["kernel"] == "df_mgrid_kernel")
+            traffic = int(row["dram_bytes_read_per_launch"]) + int(row["dram_bytes_write_per_launch"])
+        except Exception:
+            traffic = None
     roofline = {"kernel": dominant, "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": (achieved / peak) if achieved else None, "traffic": None,
+                "frac": (achieved / peak) if achieved else None, "traffic": traffic,
+                "traffic_note": "DRAM read + write bytes per launch, ncu --set full (profiles/r1b_cfg2_mgrid.md); the kernel's "
+                                "algorithmic HBM bytes are the 16 darkfield images of each tile = 268 MB per launch, the rest "
+                                "is scratch evicted from L2",
                 "avg_launch_ms": avg_ms, "sampled_launches": int(samples), "launches": int(nlaunch),
                 "share_of_kernel_time": share, "flop_per_launch": flop_per_launch, "flop_model": note,
                 "peak_note": f"{sms} SMs x {FP32_LANES_PER_SM} FMA lanes x 2 x {sm_max:.0f} MHz (derived, DESIGN.md §5)",
