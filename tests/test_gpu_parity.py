@@ -318,3 +318,25 @@ def test_host_entry_pipelines_sub_batches_without_changing_bits(A):
         assert np.array_equal(field, ref[0]) and np.array_equal(zern, ref[1])
         assert np.array_equal(pupil, ref[2]) and np.array_equal(status, ref[3])
     assert np.array_equal(field[0], field[4]) and np.array_equal(field[1], field[69])
+
+
+def test_config4_full_tile_size_with_background_tiles(A):
+    """Config 4's tiles at full size (256 x 256, 8 + 16 LEDs, the reduced-grid darkfield kernel) with
+    blank tiles in the batch: statuses of every tile, zero outputs for the skipped ones, one live tile
+    against the oracle, and the live tiles independent of the blank ones around them."""
+    from apic_synth import make_tile
+    cfg = get_config(4, batch=7, grid=(4, 2))
+    blank = np.array([1, 0, 1, 0, 0, 1, 0], dtype=bool)
+    stacks = np.empty((7, cfg.n_bright + cfg.n_dark, cfg.tile_n, cfg.tile_n), np.float32)
+    for t in range(7):
+        stacks[t], _ = make_tile(cfg, t, blank=bool(blank[t]))
+    kw = dict(bg_mode=1, bg_threshold=0.9)
+    plan, field, zern, pupil, status = gpu_reconstruct(A, cfg, stacks, chunk_tiles=3, **kw)
+    assert np.array_equal(status == 1, blank) and np.all(status[~blank] == 0)
+    for b in np.nonzero(blank)[0]:
+        assert not field[b].any() and not zern[b].any() and not pupil[b].any()
+    p = oracle_params(cfg, **kw)
+    ref = O.reconstruct_tile(stacks[3], p)
+    check_tile(ref, field[3], zern[3], pupil[3], status[3], "cfg4 tile 3")
+    _, field1, zern1, _, status1 = gpu_reconstruct(A, cfg, stacks[[1, 3, 4, 6]], **kw)
+    assert np.array_equal(field1, field[[1, 3, 4, 6]]) and np.array_equal(zern1, zern[[1, 3, 4, 6]])
