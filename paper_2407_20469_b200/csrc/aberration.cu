@@ -59,21 +59,21 @@ __global__ void __launch_bounds__(256) ab_gram(DevTables t, const float2* __rest
       const float2 q = cmulc(p1, p0);
       b = atan2f(q.y, q.x);
       w = sqrtf(p0.x * p0.x + p0.y * p0.y) * sqrtf(p1.x * p1.x + p1.y * p1.y);
-      const float* a0 = t.a_full + size_t(rr.x) * nz;
-      const float* a1 = t.a_full + size_t(rr.y) * nz;
+      const float* a0 = t.a_full + rr.x;
+      const float* a1 = t.a_full + rr.y;
       const float sw = sqrtf(w);
-      for (int j = 0; j < nz; ++j) row[j] = sw * (__ldg(&a1[j]) - __ldg(&a0[j]));
+      for (int j = 0; j < nz; ++j) row[j] = sw * (__ldg(&a1[size_t(j) * t.n_rows]) - __ldg(&a0[size_t(j) * t.n_rows]));
       row[nz] = sw * b;
       row[nz + 1] = sw;
     } else {
       const float2 p = pr[r];
       const float beta = atan2f(p.y, p.x);
       w = sqrtf(p.x * p.x + p.y * p.y);
-      const float* a = t.a_full + size_t(r) * nz;
+      const float* a = t.a_full + r;
       const float sw = sqrtf(w);
       float dot = 0.f;
       for (int j = 0; j < nz; ++j) {
-        const float aj = __ldg(&a[j]);
+        const float aj = __ldg(&a[size_t(j) * t.n_rows]);
         dot += aj * c_sh[j];
         row[j] = sw * aj;
       }

@@ -221,7 +221,14 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
   d.n_rows = int(h.row_src.size() / 2);
   d.n_grad = int(h.grad_rows.size() / 2);
   ok = ok && plan->upload(&d.row_src, h.row_src);
-  ok = ok && plan->upload(&d.a_full, h.a_full);
+  {
+    // device copy transposed to [nz][n_rows]: consecutive threads (consecutive rows) read consecutive floats
+    const size_t nr = h.a_full.size() / size_t(std::max(1, nz));
+    std::vector<float> at(h.a_full.size());
+    for (size_t r = 0; r < nr; ++r)
+      for (int j = 0; j < nz; ++j) at[size_t(j) * nr + r] = h.a_full[r * nz + j];
+    ok = ok && plan->upload(&d.a_full, at);
+  }
   ok = ok && plan->upload(&d.grad_rows, h.grad_rows);
   d.n_union = int(h.union_f.size());
   ok = ok && plan->upload(&d.union_f, h.union_f);

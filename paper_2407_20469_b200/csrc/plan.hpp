@@ -26,7 +26,7 @@ struct DevTables {
   // aberration system
   int n_rows, n_grad;
   const int32_t* row_src;        // [n_rows][2]
-  const float* a_full;           // [n_rows][nz]
+  const float* a_full;           // [nz][n_rows] (transposed on upload)
   const int32_t* grad_rows;      // [n_grad][2]
   // stitching
   int n_union;
