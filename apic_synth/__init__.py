@@ -6,5 +6,5 @@ path's tests/bench: it makes intensity stacks with the paper's forward model
 holds none of the reconstruction arithmetic.  It imports neither ``oracle`` nor
 ``paper_2407_20469_b200``.
 """
-from .configs import ApicConfig, get_config, led_kvectors, CONFIG_NAMES  # noqa: F401
+from .configs import ApicConfig, get_config, led_kvectors, plan_args, CONFIG_NAMES  # noqa: F401
 from .forward import make_tile, make_batch, TileTruth  # noqa: F401

@@ -109,3 +109,10 @@ def led_kvectors(cfg: ApicConfig) -> Tuple[np.ndarray, np.ndarray]:
             a = 2.0 * math.pi * (i + 0.5 * (r % 2)) / n
             kd.append((na / lam * math.cos(a), na / lam * math.sin(a)))
     return kb, np.asarray(kd, dtype=np.float64).reshape(-1, 2)
+
+
+def plan_args(cfg: ApicConfig) -> tuple:
+    """Positional arguments of the library's plan constructor for this recipe: (N, u, lambda, pixel, NA,
+    k_bright, k_dark, fitted Noll indices) - the optics and LED layout only, no method arithmetic."""
+    kb, kd = led_kvectors(cfg)
+    return (cfg.tile_n, cfg.upsample, cfg.wavelength_um, cfg.pixel_um, cfg.na_obj, kb, kd, tuple(cfg.noll_fit))

@@ -10,10 +10,14 @@ on (config 1 is a single tile, i.e. a latency case).  Prints ONE 
 
   value     output megapixels/s with the inputs resident in HBM (CUDA events, max over ranks)
   e2e       the same metric through apic_reconstruct_host with pinned HOST buffers (H2D + D2H inside)
-  roofline  the dominant kernel (df_cols_mul: column IFFT . p . column FFT of the darkfield CG),
-            timed live by CUDA events inside the library on the launching stream
+  roofline  the dominant kernel (df_mgrid_kernel: the darkfield CG on reduced cyclic grids), timed live by CUDA
+            events inside the library on the launching stream, against fp32 peaks MEASURED in this run
+            (apic_measure_peak: FFMA and FADD register loops, shared-memory reads)
   cpu_baseline  the fp64 oracle, as it stands, on this box's host cores, on a bounded sample
 `--impl reference` times the oracle alone (rank 0 only under torchrun).
+`--config 4` is the slide-scale streaming run: 20,000 tiles generated on the device from a seed
+(apic_synth/device.py), 40 % of them background, reconstructed in passes through apic_reconstruct_u16; every status
+flag is checked against the generator's blank mask; `--oracle-sample M` also compares M live tiles with the oracle.
 """
 from __future__ import annotations
 
@@ -39,13 +43,15 @@ FP32_LANES_PER_SM = 128          # FMA lanes per SM (4 SMSPs x 32), B200
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=0, help="timed steps (default 20; config 4: every pass of the slide)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="apic", choices=["apic", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (2 = default workload)")
     ap.add_argument("--tiles", type=int, default=0, help="tiles per step and per GPU (0 = the config's batch, capped at 64)")
     ap.add_argument("--chunk", type=int, default=0, help="apic_params.chunk_tiles (0 = library default)")
-    ap.add_argument("--df-mode", type=int, default=0, help="darkfield scheduler: 0 team kernel (reduced grids at N=256), 1 launch per phase, 2 ticket kernel, 3 team kernel on the full grid")
+    ap.add_argument("--df-mode", type=int, default=0, help="darkfield kernel: 0 team kernel (reduced grids at N=256), 3 team kernel on the full grid")
+    ap.add_argument("--pass-tiles", type=int, default=592, help="config 4: tiles per apic_reconstruct_u16 call (a step)")
+    ap.add_argument("--oracle-sample", type=int, default=0, help="config 4: live tiles compared with the fp64 oracle after the run")
     ap.add_argument("--df-team", type=int, default=0, help="apic_params.df_team: CTAs per tile of the team kernel (0 = auto)")
     ap.add_argument("--df-tol", type=float, default=-1.0, help="CG tolerance (default: the library's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -161,17 +167,64 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+# ------------------------------------------------------------------------------------ roofline helpers
+KERNEL_SOURCES = ("df_mgrid.cu", "df_team.cu", "fft_xy.cuh", "fft_core.cuh")
+
+
+def kernel_source_hash():
+    """Identifies the darkfield kernel sources an ncu capture under profiles/ was taken with (the GPU box has no .git)."""
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_2407_20469_b200", "csrc", name), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_capture(kernel, workload):
+    """Per-launch DRAM bytes and shared-memory wavefronts of `kernel` from the committed ncu --set full summary
+    (profiles/r2_ncu_kernels.csv).  A row taken with other kernel sources than the ones in the tree is refused."""
+    import csv
+    try:
+        with open(os.path.join(ROOT, "profiles", "r2_ncu_kernels.csv")) as fh:
+            rows = [r for r in csv.DictReader(fh) if r["kernel"] == kernel and r["workload"] == workload]
+    except Exception:
+        return None
+    if not rows:
+        return None
+    r = rows[-1]
+    if r["source_hash"] != kernel_source_hash():
+        return {"stale": True, "source_hash": r["source_hash"]}
+    return {"stale": False, "dram_bytes": int(r["dram_bytes_read"]) + int(r["dram_bytes_write"]),
+            "smem_wavefronts": int(r["smem_wavefronts"]), "duration_ms": float(r["duration_ms"]), "commit": r["commit"]}
+
+
+def measured_peaks(A, torch, sm_mhz_max, sms):
+    """fp32 FFMA / FADD rates and shared-memory read bandwidth measured on this device now; the derived figures
+    (unit counts x clock) beside them."""
+    fma = A.measure_peak(0) / 1e12
+    fadd = A.measure_peak(1) / 1e12
+    smem = A.measure_peak(2) / 1e12
+    return {"fp32_fma_tflops": fma, "fp32_fadd_tflops": fadd, "smem_tbs": smem,
+            "fp32_fma_tflops_derived": sms * FP32_LANES_PER_SM * 2 * sm_mhz_max * 1e6 / 1e12,
+            "smem_tbs_derived": sms * 128 * sm_mhz_max * 1e6 / 1e12,
+            "how": "apic_measure_peak: register-resident FFMA / FADD loops (8 independent accumulators, 4 x 512 threads per "
+                   "SM) and conflict-free 16-byte shared-memory loads, best of 3 after warm-up, CUDA events"}
+
+
 # ------------------------------------------------------------------------------------ product arm
 def main():
     args = parse_args()
-    from apic_synth import get_config, make_batch
+    from apic_synth import get_config, make_batch, plan_args
     cfg = get_config(args.config)
     if args.impl == "reference":
+        args.steps = args.steps or 20
         run_reference(args, cfg)
         return
     assert args.warmup >= 3, "timing rules: at least 3 warm-up steps"
     import torch
     import paper_2407_20469_b200 as A
+    from paper_2407_20469_b200.sharding import max_over_ranks, shard_tiles
     A.load()                                            # raises if libapic.so is missing: no fallback
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -189,7 +242,85 @@ def main():
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except Exception:
         pass
+    ctx = dict(args=args, cfg=cfg, torch=torch, A=A, rank=rank, world=world, local=local, dist=dist, peaks=peaks,
+               max_over_ranks=max_over_ranks, shard_tiles=shard_tiles)
+    if args.config == 4:
+        run_stream(ctx)
+    else:
+        args.steps = args.steps or 20
+        run_batch(ctx)
+    if dist:
+        dist.destroy_process_group()
 
+
+def make_sampler(local):
+    sampler = ClockSampler(str(local))
+    if os.environ.get("CUDA_VISIBLE_DEVICES"):
+        vis = os.environ["CUDA_VISIBLE_DEVICES"].split(",")
+        sampler.gpu_id = vis[local] if local < len(vis) else str(local)
+    return sampler
+
+
+def roofline_line(ctx, plan, prof, clocks, tiles, workload, step_ms, algo_hbm_bytes_per_step):
+    """The dominant kernel against the measured fp32 peaks."""
+    args, cfg, torch, A = ctx["args"], ctx["cfg"], ctx["torch"], ctx["A"]
+    peaks = ctx["peaks"]
+    sm_max = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
+    sms = torch.cuda.get_device_properties(ctx["local"]).multi_processor_count
+    mp = measured_peaks(A, torch, sm_max, sms)
+    total_kernel_ms = sum(v[0] / max(v[1], 1) * v[2] for v in prof.values())
+    dominant = max(prof, key=lambda k: prof[k][0] / max(prof[k][1], 1) * prof[k][2])
+    ms_sum, samples, nlaunch = prof[dominant]
+    avg_ms = ms_sum / max(samples, 1)
+    share = (avg_ms * nlaunch / total_kernel_ms) if total_kernel_ms else None
+    hbm_peak = peaks.get("hbm_gbs") or peaks.get("hbm_gbs_burst")
+    out = {"kernel": dominant, "avg_launch_ms": avg_ms, "sampled_launches": int(samples), "launches": int(nlaunch),
+           "share_of_kernel_time": share, "measured_peaks": mp,
+           "step_hbm": {"algorithmic_bytes_per_step": int(algo_hbm_bytes_per_step),
+                        "achieved_gbs": algo_hbm_bytes_per_step / (step_ms * 1e-3) / 1e9, "peak_gbs": hbm_peak,
+                        "frac": (algo_hbm_bytes_per_step / (step_ms * 1e-3) / 1e9 / hbm_peak) if hbm_peak else None,
+                        "note": "inputs read once + outputs written once per step, over the whole step time"}}
+    if dominant.startswith("df_"):
+        # executed work counted by the kernel itself: 5 L log2 L per L-point line transform of its strip tasks
+        # (L = N, or the per-LED reduced grid sizes 96..256 of df_mgrid.cu at N = 256); pointwise work not counted
+        flop = plan.profile_work()
+        flop_per_launch = flop / max(nlaunch, 1)
+        achieved = flop_per_launch / (avg_ms * 1e-3) / 1e12 if samples else None
+        cap = ncu_capture(dominant, workload)
+        traffic, smem_frac, cap_note = None, None, "no ncu --set full capture of this kernel and workload under profiles/"
+        if cap and cap.get("stale"):
+            cap_note = "profiles/r2_ncu_kernels.csv was captured with other kernel sources (hash mismatch): refused"
+        elif cap:
+            traffic = cap["dram_bytes"]
+            # 128 bytes per shared-memory wavefront, against the measured shared-memory read bandwidth
+            smem_frac = cap["smem_wavefronts"] * 128.0 / (cap["duration_ms"] * 1e-3) / (mp["smem_tbs"] * 1e12)
+            cap_note = f"ncu --set full at commit {cap['commit']} (profiles/r2_ncu_kernels.csv), per launch"
+        out.update({"bound": "alu", "achieved": achieved, "peak": mp["fp32_fma_tflops"], "unit": "TFLOP/s",
+                    "frac": (achieved / mp["fp32_fma_tflops"]) if achieved else None,
+                    "frac_of_fadd_peak": (achieved / mp["fp32_fadd_tflops"]) if achieved else None,
+                    "traffic": traffic, "smem_frac": smem_frac, "ncu": cap_note,
+                    "flop_per_launch": flop_per_launch,
+                    "flop_model": "nominal FFT flop executed, 5 L log2 L per L-point line transform, counted by the kernel; an "
+                                  "add-dominated radix-16 butterfly executes ~0.66 fp32 instructions per nominal flop, so the "
+                                  "instruction-issue roof in these units is ~1.5 x the FADD peak / 2 (DESIGN.md section 5)",
+                    "peak_note": "fp32 FFMA rate measured in this run (flop = 2 x FMA); FADD rate beside it"})
+    else:
+        # HBM-bound kernels (no darkfield LEDs): the whole step against the measured copy bandwidth
+        out.update({"bound": "hbm", "achieved": out["step_hbm"]["achieved_gbs"], "peak": hbm_peak, "unit": "GB/s",
+                    "frac": out["step_hbm"]["frac"], "traffic": None})
+    if args.breakdown and ctx["rank"] == 0:
+        print(f"{'kernel':22s} {'launches':>9s} {'avg us':>9s} {'est ms/step':>12s} {'share':>7s}", file=sys.stderr)
+        for k, v in sorted(prof.items(), key=lambda kv: -(kv[1][0] / max(kv[1][1], 1) * kv[1][2])):
+            est = v[0] / max(v[1], 1) * v[2]
+            print(f"{k:22s} {v[2]:9d} {1e3 * v[0] / max(v[1], 1):9.2f} {est / max(args.steps, 1):12.3f} "
+                  f"{est / max(total_kernel_ms, 1e-12):7.3f}", file=sys.stderr)
+        print(f"sum of kernel time {total_kernel_ms / max(args.steps, 1):.3f} ms/step vs step {step_ms:.3f} ms", file=sys.stderr)
+    return out
+
+
+def run_batch(ctx):
+    args, cfg, torch, A, rank, world, local, dist = (ctx[k] for k in ("args", "cfg", "torch", "A", "rank", "world", "local", "dist"))
+    from apic_synth import make_batch, plan_args
     tiles = args.tiles or min(cfg.batch, 64)
     # seeded synthetic tiles of this rank (weak scaling: every GPU gets its own `tiles` tiles); a few
     # distinct tiles are generated and repeated to fill the batch, each GPU starting at another tile
@@ -200,7 +331,7 @@ def main():
     host = np.concatenate([stacks] * reps)[:tiles]
     x = torch.from_numpy(host).cuda()
     popts = {"df_tol": args.df_tol} if args.df_tol > 0 else {}
-    plan = A.Plan.from_config(cfg, max_batch=tiles, chunk_tiles=args.chunk, df_mode=args.df_mode, df_team=args.df_team, **popts)
+    plan = A.Plan(*plan_args(cfg), max_batch=tiles, chunk_tiles=args.chunk, df_mode=args.df_mode, df_team=args.df_team, **popts)
     n, on, nz = cfg.tile_n, cfg.out_n, plan.nz
     out = (torch.empty((tiles, on, on), dtype=torch.complex64, device="cuda"),
            torch.empty((tiles, nz), dtype=torch.float32, device="cuda"),
@@ -216,12 +347,9 @@ def main():
     for _ in range(args.warmup):
         plan.reconstruct(x, out=out)
     barrier()
-    sampler = ClockSampler(str(local))
-    if os.environ.get("CUDA_VISIBLE_DEVICES"):
-        vis = os.environ["CUDA_VISIBLE_DEVICES"].split(",")
-        sampler.gpu_id = vis[local] if local < len(vis) else str(local)
+    sampler = make_sampler(local)
     sampler.start()
-    plan.profile_begin(stride=1 if args.df_mode != 1 else 4, max_samples=16384)
+    plan.profile_begin(stride=1, max_samples=16384)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches = 0
     barrier()
@@ -233,69 +361,17 @@ def main():
     barrier()
     prof = plan.profile_end()
     clocks = sampler.stop()
-    ms = e0.elapsed_time(e1)
-    if dist:
-        t = torch.tensor([ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = ctx["max_over_ranks"](e0.elapsed_time(e1), dist, device="cuda")
     status = out[3].cpu().numpy()
-    live = int((status != 1).sum())
+    n_ok = int((status == 0).sum())
+    if n_ok != tiles:
+        raise SystemExit(f"bench: {tiles - n_ok} of {tiles} tiles were not reconstructed (status {np.unique(status).tolist()}); "
+                         "the throughput of a failed step is not a result")
     mpx = world * args.steps * tiles * on * on / 1e6 / (ms / 1e3)
-
-    # ---- roofline of the dominant kernel: executed flops / CUDA-event time
     chunk = plan.info["chunk_tiles"]
-    fft_line = 5.0 * n * math.log2(n)                    # flop of one N-point complex FFT (5 N log2 N)
-    sm_max = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
-    sms = torch.cuda.get_device_properties(local).multi_processor_count
-    peak = sms * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
-    total_kernel_ms = sum(v[0] / max(v[1], 1) * v[2] for v in prof.values())
-    dominant = "df_persistent" if args.df_mode != 1 and cfg.n_dark else "df_cols_mul"
-    if not cfg.n_dark:
-        dominant = max(prof, key=lambda k: prof[k][0] / max(prof[k][1], 1) * prof[k][2])
-    ms_sum, samples, nlaunch = prof[dominant]
-    avg_ms = ms_sum / max(samples, 1)
-    if dominant == "df_persistent":
-        # executed work counted by the kernel itself: 5 L log2 L per L-point line transform of its strip tasks
-        # (L = N, or the per-LED reduced grid sizes 96..256 of df_mgrid.cu at N = 256)
-        flop = plan.profile_work()
-        flop_per_launch = flop / max(nlaunch, 1)
-        note = (f"{flop:.4g} nominal FFT flop executed (5 L log2 L per L-point line transform, counted by the kernel) "
-                f"over {nlaunch} launches; pointwise work not counted")
-    elif dominant == "df_cols_mul":
-        n_chunks = -(-tiles // chunk)
-        flop_per_launch = (2 * n * fft_line + 6.0 * n * n) * tiles / n_chunks
-        note = "N columns x (IFFT + FFT) x 5 N log2 N + complex multiply, per tile of the launch"
-    else:
-        flop_per_launch, note = None, "no flop model for this kernel"
-    achieved = flop_per_launch / (avg_ms * 1e-3) / 1e12 if (samples and flop_per_launch) else None
-    share = (avg_ms * nlaunch / total_kernel_ms) if total_kernel_ms else None
-    # DRAM bytes per launch of that kernel from the committed ncu --set full capture (same workload only)
-    traffic = None
-    if dominant == "df_persistent" and args.config == 2 and tiles == 64 and args.df_mode == 0:
-        try:
-            import csv
-            with open(os.path.join(ROOT, "profiles", "r1b_traffic_cfg2.csv")) as fh:
-                row = next(r for r in csv.DictReader(fh) if r["kernel"] == "df_mgrid_kernel")
-            traffic = int(row["dram_bytes_read_per_launch"]) + int(row["dram_bytes_write_per_launch"])
-        except Exception:
-            traffic = None
-    roofline = {"kernel": dominant, "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": (achieved / peak) if achieved else None, "traffic": traffic,
-                "traffic_note": "DRAM read + write bytes per launch, ncu --set full (profiles/r1b_cfg2_mgrid.md); the kernel's "
-                                "algorithmic HBM bytes are the 16 darkfield images of each tile = 268 MB per launch, the rest "
-                                "is scratch evicted from L2",
-                "avg_launch_ms": avg_ms, "sampled_launches": int(samples), "launches": int(nlaunch),
-                "share_of_kernel_time": share, "flop_per_launch": flop_per_launch, "flop_model": note,
-                "peak_note": f"{sms} SMs x {FP32_LANES_PER_SM} FMA lanes x 2 x {sm_max:.0f} MHz (derived, DESIGN.md §5)",
-                "hbm_peak_gbs_measured": peaks.get("hbm_gbs")}
-    if args.breakdown and rank == 0:
-        print(f"{'kernel':22s} {'launches':>9s} {'avg us':>9s} {'est ms/step':>12s} {'share':>7s}", file=sys.stderr)
-        for k, v in sorted(prof.items(), key=lambda kv: -(kv[1][0] / max(kv[1][1], 1) * kv[1][2])):
-            est = v[0] / max(v[1], 1) * v[2]
-            print(f"{k:22s} {v[2]:9d} {1e3 * v[0] / max(v[1], 1):9.2f} {est / args.steps:12.3f} "
-                  f"{est / max(total_kernel_ms, 1e-12):7.3f}", file=sys.stderr)
-        print(f"sum of kernel time {total_kernel_ms / args.steps:.3f} ms/step vs step {ms / args.steps:.3f} ms",
-              file=sys.stderr)
+    workload = f"cfg{args.config}_{tiles}tiles"
+    algo_bytes = tiles * (host[0].nbytes + on * on * 8 + n * n * 8 + nz * 4 + 4)
+    roofline = roofline_line(ctx, plan, prof, clocks, tiles, workload, ms / args.steps, algo_bytes)
 
     # ---- end to end through the host-buffer entry point (pinned memory, copies inside the timed region)
     e2e = None
@@ -307,17 +383,14 @@ def main():
         hs = torch.empty((tiles,), dtype=torch.int32).pin_memory()
         stream = torch.cuda.current_stream().cuda_stream
         plan.reconstruct_host(hx, hf, hz, hp, hs, stream)          # warm-up (allocates the staging buffers)
-        k2 = max(1, min(args.steps, 3))
+        k2 = max(1, min(args.steps, 5))
         barrier()
         t0 = time.perf_counter()
         for _ in range(k2):
             plan.reconstruct_host(hx, hf, hz, hp, hs, stream)
         torch.cuda.synchronize()
-        dt = time.perf_counter() - t0
-        if dist:
-            t = torch.tensor([dt], device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = ctx["max_over_ranks"](time.perf_counter() - t0, dist, device="cuda")
+        assert np.array_equal(hf.numpy(), out[0].cpu().numpy()), "host entry and device entry disagree"
         e2e = {"value": world * k2 * tiles * on * on / 1e6 / dt, "unit": UNIT,
                "h2d_bytes_per_step": int(hx.numel() * 4),
                "d2h_bytes_per_step": int(hf.numel() * 8 + hz.numel() * 4 + hp.numel() * 8 + hs.numel() * 4),
@@ -336,11 +409,7 @@ def main():
             for _ in range(k2):
                 plan.reconstruct_host_u16(hr, hsc, hf, hz, hp, hs, stream)
             torch.cuda.synchronize()
-            dt = time.perf_counter() - t0
-            if dist:
-                t = torch.tensor([dt], device="cuda")
-                dist.all_reduce(t, op=dist.ReduceOp.MAX)
-                dt = float(t.item())
+            dt = ctx["max_over_ranks"](time.perf_counter() - t0, dist, device="cuda")
             e2e["u16"] = {"value": world * k2 * tiles * on * on / 1e6 / dt, "unit": UNIT,
                           "h2d_bytes_per_step": int(hr.numel() * 2 + hsc.numel() * 4),
                           "api": "apic_reconstruct_host_u16 (pinned host buffers, uint16 counts + per-image scale)"}
@@ -358,14 +427,122 @@ def main():
                 "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": workload_name(cfg, tiles), "tiles_per_step_per_gpu": tiles,
+                           "distinct_tiles": n_gen, "tiles_ok": n_ok,
                            "tiles_per_s": world * args.steps * tiles / (ms / 1e3), "chunk_tiles": chunk,
-                           "live_tiles": live, "cache": "inputs larger than L2 "
+                           "cache": "inputs larger than L2 "
                            f"({host.nbytes / 1e6:.0f} MB per step vs 126 MB L2)", "parallelism": f"tiles x{world}"},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
                 "cpu_baseline": cpu}
         print(json.dumps(line), flush=True)
-    if dist:
-        dist.destroy_process_group()
+
+
+def run_stream(ctx):
+    """BASELINE.json config 4: the slide-scale streaming run.  A step = one pass of `--pass-tiles` tiles (generated on
+    the device outside the timed region, then reconstructed from uint16 counts inside it)."""
+    args, cfg, torch, A, rank, world, local, dist = (ctx[k] for k in ("args", "cfg", "torch", "A", "rank", "world", "local", "dist"))
+    from apic_synth import plan_args
+    from apic_synth.device import DeviceGenerator
+    total = args.tiles or cfg.batch
+    mine = ctx["shard_tiles"](total, rank, world)                      # contiguous scan-row ranges per GPU, no collective
+    P = max(1, min(args.pass_tiles, len(mine)))
+    passes = [(t0, min(P, mine.stop - t0)) for t0 in range(mine.start, mine.stop, P)]
+    if args.steps:
+        passes = passes[:args.steps]
+    bg = dict(bg_mode=1, bg_threshold=0.9)
+    plan = A.Plan(*plan_args(cfg), max_batch=P, chunk_tiles=args.chunk, df_team=args.df_team, **bg)
+    gen = DeviceGenerator(cfg, device=f"cuda:{local}")
+    n, on, nz = cfg.tile_n, cfg.out_n, plan.nz
+    out = (torch.empty((P, on, on), dtype=torch.complex64, device="cuda"), torch.empty((P, nz), dtype=torch.float32, device="cuda"),
+           torch.empty((P, n, n), dtype=torch.complex64, device="cuda"), torch.empty((P,), dtype=torch.int32, device="cuda"))
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    raw, scale, blank = gen.generate(*passes[0])
+    for _ in range(args.warmup):
+        plan.reconstruct_u16(raw, scale, out=tuple(o[:raw.shape[0]] for o in out))
+    barrier()
+    want = args.oracle_sample if (rank == 0 and world == 1) else 0
+    live_all = np.nonzero(~gen.blank[mine.start:mine.stop])[0] + mine.start
+    pick = set(live_all[np.linspace(0, len(live_all) - 1, want).astype(int)].tolist()) if want else set()
+    kept = []
+    sampler = make_sampler(local)
+    sampler.start()
+    plan.profile_begin(stride=1, max_samples=16384)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in passes]
+    launches, n_live, n_done, wrong, in_bytes = 0, 0, 0, 0, 0
+    barrier()
+    for k, (t0, cnt) in enumerate(passes):
+        if k:
+            raw, scale, blank = gen.generate(t0, cnt)
+        o = tuple(x[:cnt] for x in out)
+        torch.cuda.synchronize()
+        ev[k][0].record()
+        plan.reconstruct_u16(raw, scale, out=o)
+        ev[k][1].record()
+        launches += plan.last_launch_count
+        status = o[3].cpu().numpy()
+        wrong += int(np.count_nonzero((status == 1) != blank) + np.count_nonzero((status != 1) & (status != 0)))
+        n_live += int((status == 0).sum())
+        n_done += cnt
+        in_bytes += raw.numel() * 2 + scale.numel() * 4
+        for b in range(cnt):
+            if t0 + b in pick:
+                kept.append((t0 + b, (raw[b].cpu().numpy().astype(np.float32) * scale[b].cpu().numpy()[:, None, None]),
+                             o[0][b].cpu().numpy(), o[1][b].cpu().numpy()))
+    barrier()
+    prof = plan.profile_end()
+    clocks = sampler.stop()
+    ms = ctx["max_over_ranks"](sum(a.elapsed_time(b) for a, b in ev), dist, device="cuda")
+    n_live_all = ctx_sum(ctx, n_live)
+    n_done_all = ctx_sum(ctx, n_done)
+    wrong_all = ctx_sum(ctx, wrong)
+    if wrong_all:
+        raise SystemExit(f"bench --config 4: {wrong_all} status flags disagree with the generator's blank mask")
+    workload = f"cfg4_{P}tiles"
+    algo = in_bytes + n_live * (on * on * 8 + n * n * 8 + nz * 4)
+    roofline = roofline_line(ctx, plan, prof, clocks, P, workload, ms / len(passes), algo / len(passes))
+    sample = None
+    if kept:
+        from oracle import apic_oracle as O
+        p, geo, sets = oracle_setup(cfg)
+        p.bg_mode, p.bg_threshold = 1, 0.9
+        worst_f = worst_c = 0.0
+        for t, x, f, z in kept:
+            r = O.reconstruct_tile(x, p, geo=geo, sets=sets)
+            assert r.status == 0
+            worst_f = max(worst_f, float(np.linalg.norm(f - r.field) / np.linalg.norm(r.field)))
+            worst_c = max(worst_c, float(np.linalg.norm(z - r.zernike)))
+        sample = {"tiles": [k[0] for k in kept], "worst_field_rel_l2": worst_f, "worst_pupil_rad": worst_c,
+                  "within_contract": bool(worst_f <= 1e-4 and worst_c <= 1e-3)}
+    if rank == 0:
+        mpx_live = n_live_all * on * on / 1e6 / (ms / 1e3)
+        line = {"metric": METRIC, "value": mpx_live, "unit": UNIT, "n_gpus": world, "steps": len(passes), "warmup": args.warmup,
+                "ms_per_step": ms / len(passes), "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic (generated on the device from a seed, apic_synth/device.py)",
+                "config": {"workload": workload_name(cfg, P) + f"; slide of {total} tiles, {world} GPU(s)",
+                           "tiles_done": n_done_all, "tiles_live": n_live_all, "tiles_background": n_done_all - n_live_all,
+                           "status_flags_checked": n_done_all, "status_flags_wrong": 0,
+                           "value_counts": "pixels of reconstructed (non-background) tiles only",
+                           "mpx_per_s_counting_skipped_tiles": n_done_all * on * on / 1e6 / (ms / 1e3),
+                           "output_gpx_live": n_live_all * on * on / 1e9, "tiles_per_s": n_done_all / (ms / 1e3),
+                           "chunk_tiles": plan.info["chunk_tiles"], "input": "uint16 counts + per-image scale (apic_reconstruct_u16)",
+                           "cache": f"inputs larger than L2 ({raw.numel() * 2 / 1e6:.0f} MB per pass vs 126 MB L2)",
+                           "oracle_sample": sample},
+                "clocks": clocks, "e2e": None, "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": None}
+        print(json.dumps(line), flush=True)
+
+
+def ctx_sum(ctx, v):
+    dist = ctx["dist"]
+    if not dist:
+        return v
+    t = ctx["torch"].tensor([float(v)], dtype=ctx["torch"].float64, device="cuda")
+    dist.all_reduce(t)
+    return int(t.item())
 
 
 if __name__ == "__main__":

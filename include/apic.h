@@ -18,8 +18,13 @@
  * A blank object (amplitude 1, phase 0) gives I = 1 in every NA-matching image and a field = 1.
  *
  * All functions return 0 (APIC_OK) on success and a negative apic_error otherwise.  No exceptions
- * cross the boundary, there is no global state and no CPU fallback: if no CUDA device is usable the
- * calls fail with APIC_ECUDA.  A plan is not thread-safe; use one plan per stream.
+ * cross the boundary and there is no CPU fallback: if no CUDA device is usable the calls fail with
+ * APIC_ECUDA.  A plan belongs to the CUDA device that was current at apic_plan_create: its tables,
+ * workspace and kernel attributes live there, every call on the plan makes that device current for
+ * its duration (and restores the caller's), and streams passed to it must belong to that device.
+ * Plans on different devices may coexist in one process.  The only process-wide state is the
+ * per-device twiddle cache of the two test entries apic_fft2d / apic_fft2d_xy (mutex-protected) and
+ * the thread-local error strings.  A plan is not thread-safe; use one plan per stream.
  */
 #ifndef APIC_H_
 #define APIC_H_
@@ -45,7 +50,10 @@ typedef enum {
 enum {
   APIC_TILE_OK = 0,
   APIC_TILE_BACKGROUND = 1, /* skipped by the background criterion; outputs are zero          */
-  APIC_TILE_BAD_INPUT = 2,  /* a non-finite input pixel; outputs are zero                     */
+  APIC_TILE_BAD_INPUT = 2,  /* a non-finite input pixel (or scale); outputs are zero.  Negative
+                               values are NOT bad input: read noise produces them, the log clamps
+                               them (intensity_floor, R6) and the darkfield right-hand
+                               side uses them as they are (B5)                        */
   APIC_TILE_SOLVE_FAILED = 3 /* weighted phase residual of the aberration fit > 1 rad RMS (or
                                 non-finite); outputs are still written                        */
 };
@@ -72,17 +80,19 @@ typedef struct {
   float bg_threshold;
   int max_batch;         /* apic_reconstruct accepts 1..max_batch tiles; workspace is sized for
                             min(max_batch, internal chunk)                                       */
-  int chunk_tiles;       /* tiles per internal pass; 0 = chosen so that one pass's transform
-                            working set stays inside the 126 MB L2                              */
+  int chunk_tiles;       /* tiles per internal pass; 0 = chosen by the library: two tiles per SM
+                            (296 on B200) for the reduced-grid darkfield kernel (N = 256, df_mode
+                            0, whose working set is ~0.3 MB per tile), otherwise as many tiles as
+                            keep the full-grid darkfield working set (1.7 N^2 complex64 per tile)
+                            inside half of the device's L2 (queried), clamped to 8..512          */
   int df_mode;           /* darkfield scheduler: 0 = team kernel (one launch per pass covers every
                             darkfield LED; a cluster of df_team CTAs owns a tile and meets at
-                            cluster barriers between phases), 1 = one launch per phase (df_iters
-                            iterations are always enqueued), 2 = ticket-scheduled persistent task
-                            kernel (one launch per LED and pass), 3 = team kernel on the full
-                            N x N grid.  At N = 256 mode 0 runs the CG mat-vecs on per-LED
-                            reduced cyclic grids; other N: same as 3     */
-  int df_team;           /* df_mode 0 / 3: CTAs per tile, 1 | 2 | 4 | 8; 0 = chosen from the
-                            pass size (as many as the pass leaves SMs for)                      */
+                            cluster barriers between phases); at N = 256 it runs the CG mat-vecs
+                            on per-LED reduced cyclic grids.  3 = the team
+                            kernel on the full N x N grid (what other N run; kept at N = 256 as a
+                            cross-check of the reduced grids)                                   */
+  int df_team;           /* CTAs per tile, 1..8; 0 = chosen from the pass size (as many as the
+                            pass leaves resident CTA slots for)                                 */
 } apic_params;
 
 /* Fills *p with the defaults (kk_pad 1, refine_iters 3, df_iters 48, df_tol 1e-4, floor 1e-6,
@@ -143,8 +153,10 @@ int apic_reconstruct(apic_plan* plan, const float* d_intensity, int batch, float
                      float* d_zernike, float* d_pupil, int32_t* d_status, void* cuda_stream);
 
 /* Same call with HOST buffers (pinned or pageable): copies the inputs to the device, runs
- * apic_reconstruct, copies the results back and synchronises the stream before returning.
- * h_pupil may be NULL. */
+ * apic_reconstruct, copies the results back and synchronises before returning.  Batches of >= 32
+ * tiles are cut into sub-batches of >= 16 tiles that alternate between two workspace sets (the
+ * second is allocated on first use) and two compute streams, with uploads and downloads on two
+ * copy streams, so that copies in both directions overlap the kernels.  h_pupil may be NULL. */
 int apic_reconstruct_host(apic_plan* plan, const float* h_intensity, int batch, float* h_field,
                           float* h_zernike, float* h_pupil, int32_t* h_status, void* cuda_stream);
 
@@ -154,9 +166,10 @@ int apic_reconstruct_host(apic_plan* plan, const float* h_intensity, int batch, 
  *   d_raw    [batch][n_bright+n_dark][N][N] uint16, same order as d_intensity
  *   d_scale  [batch][n_bright+n_dark] float: intensity = count * scale (1 / (gain * exposure) of
  *            that frame, so that all frames are in common radiometric units, R17)
- * The conversion is fused into the S0 statistics pass (one read of the counts, one fp32 working
- * copy owned by the plan, allocated on first use: max_batch * n_img * N * N * 4 bytes); every later
- * step is the fp32 path, so the results equal apic_reconstruct on float(count) * scale bit for bit.
+ * The conversion float(count) * scale (one fp32 multiply) is fused into the loads of the three steps
+ * that read images - S0 statistics, S1 log-intensity, S8 darkfield right-hand side - so no fp32 copy
+ * of the counts exists and the input bytes read from HBM are halved; the results equal
+ * apic_reconstruct on float(count) * scale bit for bit (tested, incl. the background decision).
  * A non-finite scale makes the tile APIC_TILE_BAD_INPUT.  Other arguments as apic_reconstruct. */
 int apic_reconstruct_u16(apic_plan* plan, const uint16_t* d_raw, const float* d_scale, int batch,
                          float* d_field, float* d_zernike, float* d_pupil, int32_t* d_status,
@@ -205,9 +218,14 @@ const char* apic_profile_category_name(int cat);
 int apic_profile_begin(apic_plan* plan, int stride, int max_samples);
 int apic_profile_end(apic_plan* plan, double* ms_sum, long long* samples, long long* launches);
 /* Nominal FFT flop (5 L log2 L per executed L-point line transform, counted by the kernels
- * themselves) of the persistent darkfield kernels since apic_profile_begin (synchronises the
- * device). */
+ * themselves) of the darkfield kernels since apic_profile_begin (synchronises the device). */
 int apic_profile_work(apic_plan* plan, unsigned long long* fft_flop);
+
+/* Measured denominators for the roofline line (bench-side; not on the reconstruction path): runs a
+ * register-resident loop on the current device, timed with CUDA events on cuda_stream, and returns
+ * what = 0: fp32 FFMA rate in flop/s (2 per FMA); 1: fp32 FADD rate in flop/s (the FFT butterflies
+ * are add-dominated); 2: shared-memory read bandwidth in bytes/s (conflict-free 16-byte loads). */
+int apic_measure_peak(int what, double* per_second, void* cuda_stream);
 
 const char* apic_strerror(int err);
 const char* apic_last_cuda_error(void);

@@ -24,7 +24,7 @@ EXPORTS = ("apic_params_default", "apic_plan_create", "apic_plan_destroy", "apic
            "apic_geometry_info", "apic_geometry_dark_grids", "apic_plan_dark_sets", "apic_reconstruct", "apic_reconstruct_host", "apic_reconstruct_u16", "apic_reconstruct_host_u16",
            "apic_debug_buffer", "apic_debug_copy", "apic_fft2d", "apic_fft2d_xy", "apic_last_launch_count", "apic_strerror",
            "apic_last_cuda_error", "apic_version", "apic_profile_categories", "apic_profile_category_name",
-           "apic_profile_begin", "apic_profile_end", "apic_profile_work")
+           "apic_profile_begin", "apic_profile_end", "apic_profile_work", "apic_measure_peak")
 
 
 class ApicError(RuntimeError):
@@ -93,6 +93,7 @@ def load() -> C.CDLL:
     lib.apic_profile_end.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_longlong),
                                      C.POINTER(C.c_longlong)]
     lib.apic_profile_work.argtypes = [C.c_void_p, C.POINTER(C.c_ulonglong)]
+    lib.apic_measure_peak.argtypes = [C.c_int, C.POINTER(C.c_double), C.c_void_p]
     _lib = lib
     return lib
 
@@ -109,7 +110,7 @@ def _check(rc: int, what: str):
 def make_params(tile_n: int, upsample: int, wavelength_um: float, pixel_um: float, na_obj: float,
                 k_bright, k_dark, noll: Sequence[int], **opts):
     """Returns (ApicParams, keep-alive tuple).  ``opts``: kk_pad, refine_iters, df_iters, df_tol,
-    intensity_floor, bg_mode, bg_threshold, max_batch, chunk_tiles."""
+    intensity_floor, bg_mode, bg_threshold, max_batch, chunk_tiles, df_mode, df_team."""
     lib = load()
     p = ApicParams()
     lib.apic_params_default(C.byref(p))
@@ -165,14 +166,6 @@ class Plan:
         self.n, self.u, self.out_n = info.tile_n, info.upsample, info.out_n
         self.n_img = info.n_bright + info.n_dark
         self.nz = info.n_zernike
-
-    @classmethod
-    def from_config(cls, cfg, **opts):
-        """cfg: apic_synth.ApicConfig-like object (tile_n, upsample, optics, noll_fit)."""
-        from apic_synth.configs import led_kvectors   # input recipe only, no method arithmetic
-        kb, kd = led_kvectors(cfg)
-        return cls(cfg.tile_n, cfg.upsample, cfg.wavelength_um, cfg.pixel_um, cfg.na_obj, kb, kd,
-                   cfg.noll_fit, **opts)
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:
@@ -240,25 +233,47 @@ class Plan:
                                               status.data_ptr(), C.c_void_p(stream)), "apic_reconstruct_u16")
         return field, zern, pupil, status
 
+    def _host_ptrs(self, b, named):
+        """Checks dtype, C-contiguity and exact shape of every host buffer before its raw pointer crosses the ABI."""
+        import torch
+        np_of = {torch.float32: np.float32, torch.complex64: np.complex64, torch.int32: np.int32, torch.uint16: np.uint16}
+        out = []
+        for name, a, dtype, shape in named:
+            if a is None:
+                out.append(None)
+                continue
+            if isinstance(a, np.ndarray):
+                ok = a.dtype == dtype and a.flags["C_CONTIGUOUS"] and tuple(a.shape) == shape
+                p = a.ctypes.data
+            elif isinstance(a, torch.Tensor):
+                ok = (not a.is_cuda and np_of.get(a.dtype) == dtype and a.is_contiguous() and tuple(a.shape) == shape)
+                p = a.data_ptr()
+            else:
+                ok, p = False, None
+            if not ok:
+                raise ApicError(f"{name} must be a C-contiguous host array of dtype {np.dtype(dtype).name} and shape {shape}")
+            out.append(p)
+        return out
+
+    def _host_outputs(self, b, field, zern, pupil, status):
+        return [("field", field, np.complex64, (b, self.out_n, self.out_n)), ("zernike", zern, np.float32, (b, self.nz)),
+                ("pupil", pupil, np.complex64, (b, self.n, self.n)), ("status", status, np.int32, (b,))]
+
     def reconstruct_host_u16(self, raw, scale, field, zern, pupil, status, stream: int = 0):
         """Host buffers (numpy arrays or CPU torch tensors, ideally pinned); blocking."""
-        def ptr(a):
-            if a is None:
-                return None
-            return a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr()
-        b = raw.shape[0]
-        _check(self._lib.apic_reconstruct_host_u16(self._h, ptr(raw), ptr(scale), b, ptr(field), ptr(zern), ptr(pupil),
-                                                   ptr(status), C.c_void_p(stream)), "apic_reconstruct_host_u16")
+        b = int(raw.shape[0])
+        p = self._host_ptrs(b, [("raw", raw, np.uint16, (b, self.n_img, self.n, self.n)),
+                                ("scale", scale, np.float32, (b, self.n_img))] + self._host_outputs(b, field, zern, pupil, status))
+        _check(self._lib.apic_reconstruct_host_u16(self._h, p[0], p[1], b, p[2], p[3], p[4], p[5], C.c_void_p(stream)),
+               "apic_reconstruct_host_u16")
 
     def reconstruct_host(self, intensity, field, zern, pupil, status, stream: int = 0):
         """Host buffers (numpy arrays or CPU torch tensors, ideally pinned); blocking."""
-        def ptr(a):
-            if a is None:
-                return None
-            return a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr()
-        b = intensity.shape[0]
-        _check(self._lib.apic_reconstruct_host(self._h, ptr(intensity), b, ptr(field), ptr(zern), ptr(pupil),
-                                               ptr(status), C.c_void_p(stream)), "apic_reconstruct_host")
+        b = int(intensity.shape[0])
+        p = self._host_ptrs(b, [("intensity", intensity, np.float32, (b, self.n_img, self.n, self.n))]
+                            + self._host_outputs(b, field, zern, pupil, status))
+        _check(self._lib.apic_reconstruct_host(self._h, p[0], b, p[1], p[2], p[3], p[4], C.c_void_p(stream)),
+               "apic_reconstruct_host")
 
     def debug_buffer(self, which: int, tiles: int):
         """Stage-level buffers of the last chunk as torch tensors (copies)."""
@@ -293,6 +308,15 @@ class Plan:
     @property
     def last_launch_count(self) -> int:
         return int(self._lib.apic_last_launch_count(self._h))
+
+
+def measure_peak(what: int) -> float:
+    """apic_measure_peak on the current device: 0 fp32 FFMA flop/s, 1 fp32 FADD flop/s, 2 shared-memory bytes/s."""
+    import torch
+    v = C.c_double()
+    _check(load().apic_measure_peak(int(what), C.byref(v), C.c_void_p(torch.cuda.current_stream().cuda_stream)),
+           "apic_measure_peak")
+    return float(v.value)
 
 
 def fft2d(x, inverse: bool = False):

@@ -182,11 +182,10 @@ __global__ void __launch_bounds__(128) ab_solve(DevTables t, const float* __rest
 void launch_aberration(const DevTables& t, const Workspace& w, const LaunchCtx& c, int refine_iters,
                        float* d_zernike, int32_t* d_status) {
   const size_t sm = size_t(kGramRows) * ((t.nz + 2) | 1) * sizeof(float);
-  static bool attr = false;
-  if (!attr) {
+  if (!c.pd->attr_ab) {
     cudaFuncSetAttribute(ab_gram<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(ab_gram<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-    attr = true;
+    c.pd->attr_ab = true;
   }
   dim3 g1((t.n_rows + 255) / 256, c.chunk_tiles);
   { ProfScope ps(c, CAT_AB_PRODUCTS);

@@ -3,6 +3,8 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <map>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -26,32 +28,41 @@ bool cuda_ok(cudaError_t e, const char* what) {
 
 }  // namespace
 
+// One workspace set: everything a pass of apic_reconstruct writes.  The plan owns two; the second is
+// allocated on first use by apic_reconstruct_host so that the kernels of one sub-batch run beside the
+// copies (and the kernels) of its neighbours.
+struct WsSet {
+  Workspace ws{};
+  BatchState bs{};
+  int32_t* h_live_count = nullptr;   // pinned
+  bool ready = false;
+};
+
 struct apic_plan {
   apic_params params{};
   HostTables host;
   DevTables dev{};
+  PlanDevice pd{};
   std::vector<DarkDev> dark;
-  const DarkDev* d_dark = nullptr;   // device copy of `dark` (team kernel)
-  Workspace ws{};
-  BatchState bs{};
+  const DarkDev* d_dark = nullptr;   // device copy of `dark`
+  WsSet set[2];
+  int chunk = 1, max_unknown = 1;
   std::vector<void*> allocs;
   size_t table_bytes = 0, workspace_bytes = 0;
   int launches = 0;
   Profiler prof;
-  int32_t* h_live_count = nullptr;   // pinned
   // staging buffers of apic_reconstruct_host (grow-only)
   float *st_int = nullptr, *st_field = nullptr, *st_zern = nullptr, *st_pupil = nullptr;
   int32_t* st_status = nullptr;
   int st_batch = 0;
   bool st_has_pupil = false;
-  float* cv_int = nullptr;           // fp32 copy of a uint16 batch (apic_reconstruct_u16), allocated on first use
   uint16_t* st_raw = nullptr;        // staging of apic_reconstruct_host_u16
   float* st_scale = nullptr;
   int st_raw_batch = 0, st_int_batch = 0;
-  // apic_reconstruct_host: copy streams and per-part events (upload done, kernels done) + one for the caller's stream
-  static constexpr int kMaxParts = 4;
-  cudaStream_t copy_in = nullptr, copy_out = nullptr;
-  cudaEvent_t part_ev[2 * kMaxParts + 1] = {};
+  // apic_reconstruct_host: copy streams, a second compute stream and per-part events (upload done, kernels done)
+  static constexpr int kMaxParts = 8;
+  cudaStream_t copy_in = nullptr, copy_out = nullptr, aux = nullptr;
+  cudaEvent_t part_ev[2 * kMaxParts + 2] = {};
 
   template <class T>
   bool dalloc(T** p, size_t count, bool table) {
@@ -72,6 +83,58 @@ struct apic_plan {
     *p = q;
     return true;
   }
+  bool alloc_set(WsSet& z);
+};
+
+bool apic_plan::alloc_set(WsSet& z) {
+  if (z.ready) return true;
+  Workspace& w = z.ws;
+  const HostTables& h = host;
+  const DevTables& d = dev;
+  const size_t nn = size_t(h.n) * h.n, c = size_t(chunk);
+  const int nz = h.nz;
+  w.chunk = chunk;
+  w.max_unknown = max_unknown;
+  const int ncol = nz + 2;
+  w.gram_entries = ncol * (ncol + 1) / 2;
+  w.gram_parts = (std::max(d.n_rows, d.n_grad) + kGramRows - 1) / kGramRows;
+  const size_t n_led = std::max<size_t>(1, h.dark.size());
+  bool ok = true;
+  ok = ok && dalloc(&w.G, c * h.nb * nn, false);
+  ok = ok && dalloc(&w.S, c * d.disc_total, false);
+  ok = ok && dalloc(&w.PR, c * d.n_rows, false);
+  ok = ok && dalloc(&w.gram, c * w.gram_parts * w.gram_entries, false);
+  ok = ok && dalloc(&w.coef, c * nz, false);
+  ok = ok && dalloc(&w.ab_fail, c, false);
+  ok = ok && dalloc(&w.O, c * nn, false);
+  ok = ok && dalloc(&w.T, c * (h.dark.empty() ? 1 : nn), false);
+  ok = ok && dalloc(&w.PF, c * (h.dark.empty() ? 1 : nn), false);
+  ok = ok && dalloc(&w.TM, c * (h.dark.empty() ? 1 : nn), false);
+  ok = ok && dalloc(&w.vec_w, c * max_unknown, false);
+  ok = ok && dalloc(&w.vec_x, c * max_unknown, false);
+  ok = ok && dalloc(&w.vec_s, c * max_unknown, false);
+  ok = ok && dalloc(&w.cg_iters, c * n_led, false);
+  ok = ok && dalloc(&w.df_work, 1, false);
+  if (ok) ok = cuda_ok(cudaMemset(w.df_work, 0, sizeof(unsigned long long)), "cudaMemset");
+  ok = ok && dalloc(&w.TOUT, c * nn * h.u, false);
+  ok = ok && dalloc(&z.bs.stats, size_t(params.max_batch) * d.n_img * 3, false);
+  ok = ok && dalloc(&z.bs.live, size_t(params.max_batch), false);
+  ok = ok && dalloc(&z.bs.live_count, 1, false);
+  ok = ok && cuda_ok(cudaMallocHost(reinterpret_cast<void**>(&z.h_live_count), sizeof(int32_t)), "cudaMallocHost");
+  if (ok) ok = cuda_ok(cudaMemset(w.cg_iters, 0, c * n_led * sizeof(int32_t)), "cudaMemset");
+  z.ready = ok;
+  return ok;
+}
+
+// Makes the plan's device current for the duration of a call (function attributes, allocations and launches
+// are per device; a plan lives on the device that was current at apic_plan_create).
+struct DeviceGuard {
+  int prev = -1;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+    if (prev != dev) cudaSetDevice(dev); else prev = -1;
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 
 static void fill_info(const HostTables& h, apic_plan_info_t* info) {
@@ -152,14 +215,15 @@ int apic_geometry_dark_grids(const apic_params* p, int* mx, int* my, int cap) {
 
 int apic_plan_destroy(apic_plan* plan) {
   if (!plan) return APIC_OK;
+  DeviceGuard guard(plan->pd.device);
   for (void* q : plan->allocs) cudaFree(q);
   for (cudaEvent_t e : plan->prof.ev) cudaEventDestroy(e);
-  if (plan->h_live_count) cudaFreeHost(plan->h_live_count);
+  for (WsSet& z : plan->set) if (z.h_live_count) cudaFreeHost(z.h_live_count);
   cudaFree(plan->st_int); cudaFree(plan->st_field); cudaFree(plan->st_zern); cudaFree(plan->st_pupil);
   cudaFree(plan->st_status);
-  cudaFree(plan->cv_int); cudaFree(plan->st_raw); cudaFree(plan->st_scale);
+  cudaFree(plan->st_raw); cudaFree(plan->st_scale);
   if (plan->copy_in) {
-    cudaStreamDestroy(plan->copy_in); cudaStreamDestroy(plan->copy_out);
+    cudaStreamDestroy(plan->copy_in); cudaStreamDestroy(plan->copy_out); cudaStreamDestroy(plan->aux);
     for (cudaEvent_t e : plan->part_ev) if (e) cudaEventDestroy(e);
   }
   delete plan;
@@ -176,6 +240,9 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
   }
   apic_plan* plan = new (std::nothrow) apic_plan;
   if (!plan) return APIC_ENOMEM;
+  cudaGetDevice(&plan->pd.device);
+  cudaDeviceGetAttribute(&plan->pd.sms, cudaDevAttrMultiProcessorCount, plan->pd.device);
+  cudaDeviceGetAttribute(&plan->pd.l2_bytes, cudaDevAttrL2CacheSize, plan->pd.device);
   std::string err;
   if (!build_geometry(*p, plan->host, err)) {
     g_plan_err = err;
@@ -238,7 +305,7 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
   d.n_pupil = int(h.pupil_idx.size());
   ok = ok && plan->upload(&d.pupil_idx, h.pupil_idx);
   ok = ok && plan->upload(&d.pupil_zern, h.pupil_zern);
-  int max_eq = 1, max_unknown = 1, dot_parts = 1;
+  int max_unknown = 1;
   for (const DarkLed& L : h.dark) {
     DarkDev q{};
     q.n_unknown = L.n_unknown; q.n_disc = L.n_disc; q.n_eq = L.n_eq;
@@ -254,56 +321,29 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
     ok = ok && plan->upload(&q.dmap_m, L.dmap_m);
     ok = ok && plan->upload(&q.qmask_m, L.qmask_m);
     plan->dark.push_back(q);
-    max_eq = std::max(max_eq, L.n_eq);
     max_unknown = std::max(max_unknown, L.n_unknown);
-    dot_parts = std::max(dot_parts, (L.u_nrow + strip_lines(n) - 1) / strip_lines(n));
   }
   ok = ok && plan->upload(&plan->d_dark, plan->dark);
-  // ---- workspace
-  Workspace& w = plan->ws;
+  // ---- workspace: tiles per internal pass
   const size_t nn = size_t(n) * n;
   int chunk = p->chunk_tiles;
   if (chunk <= 0) {
-    // darkfield CG working set per tile: T rows in use (<= 2/3 N) + p (N^2)  ~ 1.7 N^2 complex64
-    const double per_tile = 1.7 * double(nn) * sizeof(float2);
-    chunk = int(64.0e6 / per_tile);
-    chunk = std::max(8, std::min(chunk, 512));
+    if (n == 256 && p->df_mode == 0 && !h.dark.empty()) {
+      // reduced-grid darkfield kernel: its CG working set is ~0.3 MB per tile (TM + p_M on grids of 15-20 k bins),
+      // so the pass is sized for the kernel's scheduler instead: up to two tiles per SM (one CTA per tile)
+      chunk = 2 * std::max(1, plan->pd.sms);
+    } else {
+      // full-grid darkfield CG working set per tile: T rows in use (<= 2/3 N) + p (N^2) ~ 1.7 N^2 complex64; a pass
+      // is sized to half of this device's L2
+      const double per_tile = 1.7 * double(nn) * sizeof(float2);
+      chunk = int(0.5 * double(std::max(plan->pd.l2_bytes, 32 << 20)) / per_tile);
+      chunk = std::max(8, std::min(chunk, 512));
+    }
   }
   chunk = std::max(1, std::min(chunk, p->max_batch));
-  w.chunk = chunk;
-  w.max_eq = max_eq; w.max_unknown = max_unknown; w.dot_parts = dot_parts;
-  const int ncol = nz + 2;
-  w.gram_entries = ncol * (ncol + 1) / 2;
-  w.gram_parts = (std::max(d.n_rows, d.n_grad) + kGramRows - 1) / kGramRows;
-  const size_t c = size_t(chunk);
-  ok = ok && plan->dalloc(&w.G, c * h.nb * nn, false);
-  ok = ok && plan->dalloc(&w.S, c * d.disc_total, false);
-  ok = ok && plan->dalloc(&w.PR, c * d.n_rows, false);
-  ok = ok && plan->dalloc(&w.gram, c * w.gram_parts * w.gram_entries, false);
-  ok = ok && plan->dalloc(&w.coef, c * nz, false);
-  ok = ok && plan->dalloc(&w.ab_fail, c, false);
-  ok = ok && plan->dalloc(&w.O, c * nn, false);
-  ok = ok && plan->dalloc(&w.T, c * nn, false);
-  ok = ok && plan->dalloc(&w.PF, c * nn, false);
-  ok = ok && plan->dalloc(&w.TM, c * (h.dark.empty() ? 1 : nn), false);
-  ok = ok && plan->dalloc(&w.vec_d, c * max_eq, false);
-  ok = ok && plan->dalloc(&w.vec_x, c * max_unknown, false);
-  ok = ok && plan->dalloc(&w.vec_s, c * max_unknown, false);
-  ok = ok && plan->dalloc(&w.vec_p, c * max_unknown, false);
-  ok = ok && plan->dalloc(&w.vec_w, c * max_unknown, false);
-  ok = ok && plan->dalloc(&w.dot_part, c * dot_parts, false);
-  ok = ok && plan->dalloc(&w.cg_scal, c * 4, false);
-  ok = ok && plan->dalloc(&w.cg_done, c, false);
-  ok = ok && plan->dalloc(&w.cg_iters, c * std::max<size_t>(1, h.dark.size()), false);
-  ok = ok && plan->dalloc(&w.df_sync, c + 2, false);
-  ok = ok && plan->dalloc(&w.df_work, 1, false);
-  if (ok) ok = cuda_ok(cudaMemset(w.df_work, 0, sizeof(unsigned long long)), "cudaMemset");
-  ok = ok && plan->dalloc(&w.TOUT, c * nn * h.u, false);
-  ok = ok && plan->dalloc(&plan->bs.stats, size_t(p->max_batch) * d.n_img * 3, false);
-  ok = ok && plan->dalloc(&plan->bs.live, size_t(p->max_batch), false);
-  ok = ok && plan->dalloc(&plan->bs.live_count, 1, false);
-  ok = ok && cuda_ok(cudaMallocHost(reinterpret_cast<void**>(&plan->h_live_count), sizeof(int32_t)), "cudaMallocHost");
-  if (ok) ok = cuda_ok(cudaMemset(w.cg_iters, 0, c * std::max<size_t>(1, h.dark.size()) * sizeof(int32_t)), "cudaMemset");
+  plan->chunk = chunk;
+  plan->max_unknown = max_unknown;
+  ok = ok && plan->alloc_set(plan->set[0]);
   if (!ok) {
     const bool oom = g_cuda_err.find("out of memory") != std::string::npos;
     apic_plan_destroy(plan);
@@ -316,7 +356,7 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
 int apic_plan_info(const apic_plan* plan, apic_plan_info_t* info) {
   if (!plan || !info) return APIC_EINVAL;
   fill_info(plan->host, info);
-  info->chunk_tiles = plan->ws.chunk;
+  info->chunk_tiles = plan->chunk;
   info->table_bytes = plan->table_bytes;
   info->workspace_bytes = plan->workspace_bytes;
   return APIC_OK;
@@ -332,61 +372,47 @@ int apic_plan_dark_sets(const apic_plan* plan, int* led, int* n_unknown, int* n_
   return APIC_OK;
 }
 
-// The whole path.  Either d_intensity (fp32) or d_raw + d_scale (uint16 counts and the per-image factor that
-// turns them into radiometric units) is given; the uint16 form is converted inside the S0 statistics pass.
-static int reconstruct_impl(apic_plan* plan, const float* d_intensity, const uint16_t* d_raw, const float* d_scale, int batch,
-                            float* d_field, float* d_zernike, float* d_pupil, int32_t* d_status, void* cuda_stream) {
-  if (!plan || !(d_intensity || (d_raw && d_scale)) || !d_field || !d_zernike || !d_status) return APIC_EINVAL;
+// The whole path on workspace set `zi`.  `src` holds either fp32 intensities or uint16 counts + per-image scale;
+// the uint16 form is converted in the loads of S0, S1 and S8 (no fp32 working copy).
+static int reconstruct_impl(apic_plan* plan, int zi, const ImgSrc& src, int batch, float* d_field, float* d_zernike,
+                            float* d_pupil, int32_t* d_status, cudaStream_t s) {
+  if (!plan || !(src.f32 || (src.u16 && src.scale)) || !d_field || !d_zernike || !d_status) return APIC_EINVAL;
   if (batch < 1 || batch > plan->params.max_batch) return APIC_EBATCH;
-  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-  if (d_raw && !plan->cv_int) {
-    const size_t bytes = size_t(plan->params.max_batch) * plan->dev.n_img * plan->dev.n * plan->dev.n * sizeof(float);
-    if (!cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->cv_int), bytes), "cudaMalloc uint16 conversion buffer")) return APIC_ENOMEM;
-    plan->workspace_bytes += bytes;
-  }
+  WsSet& z = plan->set[zi];
+  if (!z.ready && !plan->alloc_set(z)) return APIC_ENOMEM;
   const DevTables& t = plan->dev;
-  const Workspace& w = plan->ws;
+  const Workspace& w = z.ws;
   const apic_params& p = plan->params;
-  plan->launches = 0;
+  if (zi == 0) plan->launches = 0;
   cudaGetLastError();
   // S0: statistics, status, list of tiles to reconstruct
   {
-    LaunchCtx c{s, &plan->launches, &plan->prof, plan->bs.live, plan->bs.live_count, 0, batch};
-    if (d_raw) {
-      launch_image_stats_u16(t, d_raw, d_scale, plan->cv_int, batch, plan->bs.stats, c);
-      d_intensity = plan->cv_int;
-    } else {
-      launch_image_stats(t, d_intensity, batch, plan->bs.stats, c);
-    }
-    launch_tile_status(t, plan->bs.stats, batch, p.bg_mode, p.bg_threshold, d_status, plan->bs.live,
-                       plan->bs.live_count, c);
+    LaunchCtx c{s, &plan->launches, &plan->prof, z.bs.live, z.bs.live_count, 0, batch, &plan->pd};
+    launch_image_stats(t, src, batch, z.bs.stats, c);
+    launch_tile_status(t, z.bs.stats, batch, p.bg_mode, p.bg_threshold, d_status, z.bs.live, z.bs.live_count, c);
     launch_zero_dead(t, d_status, batch, d_field, d_zernike, d_pupil, c);
   }
   if (d_pupil) cudaMemsetAsync(d_pupil, 0, size_t(batch) * t.n * t.n * sizeof(float2), s);
   int n_live = batch;
   if (p.bg_mode != 0) {
-    cudaMemcpyAsync(plan->h_live_count, plan->bs.live_count, sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+    cudaMemcpyAsync(z.h_live_count, z.bs.live_count, sizeof(int32_t), cudaMemcpyDeviceToHost, s);
     if (!cuda_ok(cudaStreamSynchronize(s), "background pass")) return APIC_ECUDA;
-    n_live = *plan->h_live_count;
+    n_live = *z.h_live_count;
   }
   const int n_dark_used = int(plan->dark.size());
   // balanced passes: ceil(n_live / chunk) passes of (almost) equal size
   const int n_pass = (n_live + w.chunk - 1) / w.chunk;
   const int per_pass = n_pass ? (n_live + n_pass - 1) / n_pass : 0;
   for (int c0 = 0; c0 < n_live; c0 += per_pass) {
-    LaunchCtx c{s, &plan->launches, &plan->prof, plan->bs.live, plan->bs.live_count, c0,
-                std::min(per_pass, n_live - c0)};
-    launch_kk(t, w, c, d_intensity, plan->bs.stats, p.intensity_floor);                       // S1-S5
+    LaunchCtx c{s, &plan->launches, &plan->prof, z.bs.live, z.bs.live_count, c0, std::min(per_pass, n_live - c0),
+                &plan->pd};
+    launch_kk(t, w, c, src, z.bs.stats, p.intensity_floor);                                   // S1-S5
     launch_aberration(t, w, c, p.refine_iters, d_zernike, d_status);                          // S6
     launch_stitch(t, w, c);                                                                   // S7
     if (p.df_mode == 0 && t.n == 256)                                                         // S8-S10
-      launch_darkfield_mgrid(t, plan->d_dark, n_dark_used, w, c, d_intensity, p.df_iters, p.df_tol, p.df_team);
-    else if (p.df_mode == 0 || p.df_mode == 3)
-      launch_darkfield_team(t, plan->d_dark, n_dark_used, w, c, d_intensity, p.df_iters, p.df_tol, p.df_team);
+      launch_darkfield_mgrid(t, plan->d_dark, n_dark_used, w, c, src, p.df_iters, p.df_tol, p.df_team);
     else
-      for (int k = 0; k < n_dark_used; ++k)
-        launch_darkfield_led(t, plan->dark[k], k, std::max(1, n_dark_used), w, c, d_intensity, p.df_iters, p.df_tol,
-                             p.df_mode);
+      launch_darkfield_team(t, plan->d_dark, n_dark_used, w, c, src, p.df_iters, p.df_tol, p.df_team);
     launch_output(t, w, c, d_field, d_pupil);                                                 // S10
   }
   if (!cuda_ok(cudaGetLastError(), "apic_reconstruct launch")) return APIC_ECUDA;
@@ -395,14 +421,18 @@ static int reconstruct_impl(apic_plan* plan, const float* d_intensity, const uin
 
 int apic_reconstruct(apic_plan* plan, const float* d_intensity, int batch, float* d_field, float* d_zernike,
                      float* d_pupil, int32_t* d_status, void* cuda_stream) {
-  if (!d_intensity) return APIC_EINVAL;
-  return reconstruct_impl(plan, d_intensity, nullptr, nullptr, batch, d_field, d_zernike, d_pupil, d_status, cuda_stream);
+  if (!plan || !d_intensity) return APIC_EINVAL;
+  DeviceGuard guard(plan->pd.device);
+  return reconstruct_impl(plan, 0, ImgSrc{d_intensity, nullptr, nullptr}, batch, d_field, d_zernike, d_pupil, d_status,
+                          static_cast<cudaStream_t>(cuda_stream));
 }
 
 int apic_reconstruct_u16(apic_plan* plan, const uint16_t* d_raw, const float* d_scale, int batch, float* d_field,
                          float* d_zernike, float* d_pupil, int32_t* d_status, void* cuda_stream) {
-  if (!d_raw || !d_scale) return APIC_EINVAL;
-  return reconstruct_impl(plan, nullptr, d_raw, d_scale, batch, d_field, d_zernike, d_pupil, d_status, cuda_stream);
+  if (!plan || !d_raw || !d_scale) return APIC_EINVAL;
+  DeviceGuard guard(plan->pd.device);
+  return reconstruct_impl(plan, 0, ImgSrc{nullptr, d_raw, d_scale}, batch, d_field, d_zernike, d_pupil, d_status,
+                          static_cast<cudaStream_t>(cuda_stream));
 }
 
 // Host-buffer form of both entries: H2D, reconstruct, D2H, one synchronisation.
@@ -416,8 +446,8 @@ int apic_reconstruct_host(apic_plan* plan, const float* h_intensity, int batch, 
   return reconstruct_host_impl(plan, h_intensity, nullptr, nullptr, batch, h_field, h_zernike, h_pupil, h_status, cuda_stream);
 }
 
-int apic_reconstruct_host_u16(apic_plan* plan, const uint16_t* h_raw, const float* h_scale, int batch, float* h_field,
-                              float* h_zernike, float* h_pupil, int32_t* h_status, void* cuda_stream) {
+int apic_reconstruct_host_u16(apic_plan* plan, const uint16_t* h_raw, const float* h_scale, int batch,
+                              float* h_field, float* h_zernike, float* h_pupil, int32_t* h_status, void* cuda_stream) {
   if (!h_raw || !h_scale) return APIC_EINVAL;
   return reconstruct_host_impl(plan, nullptr, h_raw, h_scale, batch, h_field, h_zernike, h_pupil, h_status, cuda_stream);
 }
@@ -427,6 +457,7 @@ static int reconstruct_host_impl(apic_plan* plan, const float* h_intensity, cons
                                  void* cuda_stream) {
   if (!plan || !h_field || !h_zernike || !h_status) return APIC_EINVAL;
   if (batch < 1 || batch > plan->params.max_batch) return APIC_EBATCH;
+  DeviceGuard guard(plan->pd.device);
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   const DevTables& t = plan->dev;
   const size_t nn = size_t(t.n) * t.n, on = size_t(t.n) * t.u;
@@ -461,22 +492,27 @@ static int reconstruct_host_impl(apic_plan* plan, const float* h_intensity, cons
     if (!cuda_ok(cudaMalloc(reinterpret_cast<void**>(&plan->st_int), n_px * sizeof(float)), "cudaMalloc staging")) return APIC_ENOMEM;
     plan->st_int_batch = batch;
   }
+  constexpr int kEv = 2 * apic_plan::kMaxParts;
   if (!plan->copy_in) {
     bool ok = cuda_ok(cudaStreamCreateWithFlags(&plan->copy_in, cudaStreamNonBlocking), "cudaStreamCreate") &&
-              cuda_ok(cudaStreamCreateWithFlags(&plan->copy_out, cudaStreamNonBlocking), "cudaStreamCreate");
-    for (int k = 0; ok && k < 2 * apic_plan::kMaxParts + 1; ++k)
+              cuda_ok(cudaStreamCreateWithFlags(&plan->copy_out, cudaStreamNonBlocking), "cudaStreamCreate") &&
+              cuda_ok(cudaStreamCreateWithFlags(&plan->aux, cudaStreamNonBlocking), "cudaStreamCreate");
+    for (int k = 0; ok && k < kEv + 2; ++k)
       ok = cuda_ok(cudaEventCreateWithFlags(&plan->part_ev[k], cudaEventDisableTiming), "cudaEventCreate");
     if (!ok) return APIC_ECUDA;
   }
-  // Sub-batches of >= 32 tiles (a smaller pass leaves the darkfield teams too few tiles to fill the GPU): the
-  // upload of part i+1 and the download of part i-1 run on their own streams beside the kernels of part i.
-  // Results do not depend on the split (a tile's result is independent of its batch; tested).
-  const int parts = std::max(1, std::min(apic_plan::kMaxParts, batch / 32));
+  // Sub-batches of >= 16 tiles alternate between the plan's two workspace sets and two compute streams (the caller's
+  // and one of the plan's), so that the kernels of part k run beside those of part k+1 and beside the upload of the
+  // parts after it and the download of the parts before it.  Results do not depend on the split (a tile's result is
+  // independent of its batch; tested).
+  const int parts = std::max(1, std::min(apic_plan::kMaxParts, batch / 16));
+  if (parts > 1 && !plan->alloc_set(plan->set[1])) return APIC_ENOMEM;
   const int per = (batch + parts - 1) / parts;
   const size_t img_px = size_t(t.n_img) * nn;
-  cudaEventRecord(plan->part_ev[2 * apic_plan::kMaxParts], s);                 // earlier work on the caller's stream
-  cudaStreamWaitEvent(plan->copy_in, plan->part_ev[2 * apic_plan::kMaxParts], 0);
-  cudaStreamWaitEvent(plan->copy_out, plan->part_ev[2 * apic_plan::kMaxParts], 0);
+  cudaEventRecord(plan->part_ev[kEv], s);                                      // earlier work on the caller's stream
+  cudaStreamWaitEvent(plan->copy_in, plan->part_ev[kEv], 0);
+  cudaStreamWaitEvent(plan->copy_out, plan->part_ev[kEv], 0);
+  cudaStreamWaitEvent(plan->aux, plan->part_ev[kEv], 0);
   for (int k = 0, b0 = 0; b0 < batch; ++k, b0 += per) {
     const int nb = std::min(per, batch - b0);
     if (h_raw) {
@@ -490,29 +526,36 @@ static int reconstruct_host_impl(apic_plan* plan, const float* h_intensity, cons
     }
     cudaEventRecord(plan->part_ev[2 * k], plan->copy_in);
   }
-  for (int k = 0, b0 = 0; b0 < batch; ++k, b0 += per) {
+  int rc = APIC_OK;
+  for (int k = 0, b0 = 0; b0 < batch && rc == APIC_OK; ++k, b0 += per) {
     const int nb = std::min(per, batch - b0);
-    cudaStreamWaitEvent(s, plan->part_ev[2 * k], 0);
+    const int zi = k & 1;
+    cudaStream_t ks = zi ? plan->aux : s;
+    cudaStreamWaitEvent(ks, plan->part_ev[2 * k], 0);
     float* f = plan->st_field + size_t(b0) * on * on * 2;
     float* z = plan->st_zern + size_t(b0) * t.nz;
     float* pu = h_pupil ? plan->st_pupil + size_t(b0) * nn * 2 : nullptr;
     int32_t* st = plan->st_status + b0;
-    const int rc = h_raw ? apic_reconstruct_u16(plan, plan->st_raw + b0 * img_px, plan->st_scale + size_t(b0) * t.n_img, nb, f, z, pu, st, s)
-                         : apic_reconstruct(plan, plan->st_int + b0 * img_px, nb, f, z, pu, st, s);
-    if (rc != APIC_OK) {
-      cudaStreamSynchronize(plan->copy_in); cudaStreamSynchronize(plan->copy_out); cudaStreamSynchronize(s);
-      return rc;
-    }
-    cudaEventRecord(plan->part_ev[2 * k + 1], s);
+    const ImgSrc src = h_raw ? ImgSrc{nullptr, plan->st_raw + b0 * img_px, plan->st_scale + size_t(b0) * t.n_img}
+                             : ImgSrc{plan->st_int + b0 * img_px, nullptr, nullptr};
+    rc = reconstruct_impl(plan, zi, src, nb, f, z, pu, st, ks);
+    if (rc != APIC_OK) break;
+    cudaEventRecord(plan->part_ev[2 * k + 1], ks);
     cudaStreamWaitEvent(plan->copy_out, plan->part_ev[2 * k + 1], 0);
     cudaMemcpyAsync(h_field + size_t(b0) * on * on * 2, f, size_t(nb) * on * on * 2 * sizeof(float), cudaMemcpyDeviceToHost, plan->copy_out);
     cudaMemcpyAsync(h_zernike + size_t(b0) * t.nz, z, size_t(nb) * t.nz * sizeof(float), cudaMemcpyDeviceToHost, plan->copy_out);
     if (h_pupil) cudaMemcpyAsync(h_pupil + size_t(b0) * nn * 2, pu, size_t(nb) * nn * 2 * sizeof(float), cudaMemcpyDeviceToHost, plan->copy_out);
     cudaMemcpyAsync(h_status + b0, st, size_t(nb) * sizeof(int32_t), cudaMemcpyDeviceToHost, plan->copy_out);
   }
-  if (!cuda_ok(cudaStreamSynchronize(plan->copy_out), "apic_reconstruct_host")) return APIC_ECUDA;
-  if (!cuda_ok(cudaStreamSynchronize(s), "apic_reconstruct_host")) return APIC_ECUDA;
-  return APIC_OK;
+  // the caller's stream also ends after the plan's second compute stream
+  cudaEventRecord(plan->part_ev[kEv + 1], plan->aux);
+  cudaStreamWaitEvent(s, plan->part_ev[kEv + 1], 0);
+  bool ok = cuda_ok(cudaStreamSynchronize(plan->copy_in), "apic_reconstruct_host");
+  ok = cuda_ok(cudaStreamSynchronize(plan->copy_out), "apic_reconstruct_host") && ok;
+  ok = cuda_ok(cudaStreamSynchronize(plan->aux), "apic_reconstruct_host") && ok;
+  ok = cuda_ok(cudaStreamSynchronize(s), "apic_reconstruct_host") && ok;
+  if (rc != APIC_OK) return rc;
+  return ok ? APIC_OK : APIC_ECUDA;
 }
 
 int apic_debug_buffer(const apic_plan* plan, int which, void** d_ptr, size_t* bytes_per_tile) {
@@ -520,11 +563,11 @@ int apic_debug_buffer(const apic_plan* plan, int which, void** d_ptr, size_t* by
   const DevTables& t = plan->dev;
   switch (which) {
     case APIC_DBG_SUBSPECTRA:
-      *d_ptr = plan->ws.S; *bytes_per_tile = size_t(t.disc_total) * sizeof(float2); return APIC_OK;
+      *d_ptr = plan->set[0].ws.S; *bytes_per_tile = size_t(t.disc_total) * sizeof(float2); return APIC_OK;
     case APIC_DBG_OBJECT_SPECTRUM:
-      *d_ptr = plan->ws.O; *bytes_per_tile = size_t(t.n) * t.n * sizeof(float2); return APIC_OK;
+      *d_ptr = plan->set[0].ws.O; *bytes_per_tile = size_t(t.n) * t.n * sizeof(float2); return APIC_OK;
     case APIC_DBG_DF_ITERS:
-      *d_ptr = plan->ws.cg_iters; *bytes_per_tile = std::max<size_t>(1, plan->dark.size()) * sizeof(int32_t); return APIC_OK;
+      *d_ptr = plan->set[0].ws.cg_iters; *bytes_per_tile = std::max<size_t>(1, plan->dark.size()) * sizeof(int32_t); return APIC_OK;
   }
   return APIC_EINVAL;
 }
@@ -534,24 +577,38 @@ int apic_debug_copy(const apic_plan* plan, int which, void* d_dst, int tiles, vo
   size_t bytes = 0;
   const int rc = apic_debug_buffer(plan, which, &src, &bytes);
   if (rc != APIC_OK) return rc;
-  if (!d_dst || tiles < 1 || tiles > plan->ws.chunk) return APIC_EINVAL;
+  if (!d_dst || tiles < 1 || tiles > plan->chunk) return APIC_EINVAL;
   if (!cuda_ok(cudaMemcpyAsync(d_dst, src, bytes * tiles, cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(cuda_stream)),
                "apic_debug_copy"))
     return APIC_ECUDA;
   return APIC_OK;
 }
 
+// Twiddle tables of the two test entries below, one set per device (allocated on first use, never freed).
+namespace {
+std::mutex g_tw_mutex;
+std::map<std::pair<int, int>, float2*> g_tw_cache;     // (device, table id) -> device pointer
+const float2* cached_twiddles(int table, const std::vector<float2>& host) {
+  int dev = 0;
+  cudaGetDevice(&dev);
+  std::lock_guard<std::mutex> lock(g_tw_mutex);
+  auto it = g_tw_cache.find({dev, table});
+  if (it != g_tw_cache.end()) return it->second;
+  float2* q = nullptr;
+  if (!cuda_ok(cudaMalloc(reinterpret_cast<void**>(&q), host.size() * sizeof(float2)), "cudaMalloc")) return nullptr;
+  if (!cuda_ok(cudaMemcpy(q, host.data(), host.size() * sizeof(float2), cudaMemcpyHostToDevice), "cudaMemcpy")) return nullptr;
+  g_tw_cache[{dev, table}] = q;
+  return q;
+}
+}  // namespace
+
 int apic_fft2d(float* d_data, int n, int batch, int inverse, void* cuda_stream) {
   if (!d_data || batch < 1 || !(n == 64 || n == 128 || n == 256 || n == 512)) return APIC_EINVAL;
-  static float2* tw_cache[4] = {nullptr, nullptr, nullptr, nullptr};
-  const int slot = n == 64 ? 0 : n == 128 ? 1 : n == 256 ? 2 : 3;
-  if (!tw_cache[slot]) {
-    std::vector<float2> tw;
-    build_twiddles(n, tw);
-    if (!cuda_ok(cudaMalloc(reinterpret_cast<void**>(&tw_cache[slot]), tw.size() * sizeof(float2)), "cudaMalloc")) return APIC_ECUDA;
-    if (!cuda_ok(cudaMemcpy(tw_cache[slot], tw.data(), tw.size() * sizeof(float2), cudaMemcpyHostToDevice), "cudaMemcpy")) return APIC_ECUDA;
-  }
-  launch_fft2d(reinterpret_cast<float2*>(d_data), n, batch, inverse != 0, tw_cache[slot], static_cast<cudaStream_t>(cuda_stream));
+  std::vector<float2> tw;
+  build_twiddles(n, tw);
+  const float2* d_tw = cached_twiddles(n, tw);
+  if (!d_tw) return APIC_ECUDA;
+  launch_fft2d(reinterpret_cast<float2*>(d_data), n, batch, inverse != 0, d_tw, static_cast<cudaStream_t>(cuda_stream));
   if (!cuda_ok(cudaGetLastError(), "apic_fft2d")) return APIC_ECUDA;
   return APIC_OK;
 }
@@ -559,16 +616,13 @@ int apic_fft2d(float* d_data, int n, int batch, int inverse, void* cuda_stream) 
 int apic_fft2d_xy(float* d_data, int mx, int my, int batch, int mode, void* cuda_stream) {
   auto okl = [](int l) { return l == 96 || l == 128 || l == 160 || l == 192 || l == 256; };
   if (!d_data || batch < 1 || !okl(mx) || !okl(my) || mode < 0 || mode > 3) return APIC_EINVAL;
-  static float2* tw = nullptr;
-  if (!tw) {
-    std::vector<float2> txy, one;
-    for (int r1 : {6, 8, 10, 12, 16}) {
-      build_twiddles_xy(r1, one);
-      txy.insert(txy.end(), one.begin(), one.end());
-    }
-    if (!cuda_ok(cudaMalloc(reinterpret_cast<void**>(&tw), txy.size() * sizeof(float2)), "cudaMalloc")) return APIC_ECUDA;
-    if (!cuda_ok(cudaMemcpy(tw, txy.data(), txy.size() * sizeof(float2), cudaMemcpyHostToDevice), "cudaMemcpy")) return APIC_ECUDA;
+  std::vector<float2> txy, one;
+  for (int r1 : {6, 8, 10, 12, 16}) {
+    build_twiddles_xy(r1, one);
+    txy.insert(txy.end(), one.begin(), one.end());
   }
+  const float2* tw = cached_twiddles(0, txy);
+  if (!tw) return APIC_ECUDA;
   if (launch_fft2d_xy(reinterpret_cast<float2*>(d_data), mx, my, batch, mode, tw, static_cast<cudaStream_t>(cuda_stream)))
     return APIC_EINVAL;
   if (!cuda_ok(cudaGetLastError(), "apic_fft2d_xy")) return APIC_ECUDA;
@@ -579,9 +633,7 @@ int apic_last_launch_count(const apic_plan* plan) { return plan ? plan->launches
 
 static const char* kCatNames[CAT_COUNT] = {
     "stats_status", "kk_log_rowfft", "kk_col_mask", "kk_row_exp", "kk_col_gather", "ab_pair_products", "ab_gram",
-    "ab_solve", "stitch", "df_build_p_rows", "df_cols_p", "df_rows_rhs", "df_rows_q", "df_cols_mul",
-    "df_rows_u_scatter", "df_rows_u_gather", "df_cg_vector", "df_extend", "out_rows", "out_cols", "pupil",
-    "df_persistent"};
+    "ab_solve", "stitch", "out_rows", "out_cols", "pupil", "df_mgrid_kernel", "df_team_kernel"};
 
 int apic_profile_categories(void) { return CAT_COUNT; }
 const char* apic_profile_category_name(int cat) { return (cat >= 0 && cat < CAT_COUNT) ? kCatNames[cat] : ""; }
@@ -599,15 +651,20 @@ int apic_profile_begin(apic_plan* plan, int stride, int max_samples) {
   pr.stride = stride;
   for (long long& v : pr.launches) v = 0;
   pr.on = true;
-  if (!cuda_ok(cudaMemset(plan->ws.df_work, 0, sizeof(unsigned long long)), "cudaMemset")) return APIC_ECUDA;
+  for (WsSet& z : plan->set)
+    if (z.ready && !cuda_ok(cudaMemset(z.ws.df_work, 0, sizeof(unsigned long long)), "cudaMemset")) return APIC_ECUDA;
   return APIC_OK;
 }
 
 int apic_profile_work(apic_plan* plan, unsigned long long* line_transforms) {
   if (!plan || !line_transforms) return APIC_EINVAL;
-  if (!cuda_ok(cudaMemcpy(line_transforms, plan->ws.df_work, sizeof(unsigned long long), cudaMemcpyDeviceToHost),
-               "apic_profile_work"))
-    return APIC_ECUDA;
+  *line_transforms = 0;
+  for (WsSet& z : plan->set) {
+    unsigned long long v = 0;
+    if (z.ready && !cuda_ok(cudaMemcpy(&v, z.ws.df_work, sizeof v, cudaMemcpyDeviceToHost), "apic_profile_work"))
+      return APIC_ECUDA;
+    *line_transforms += v;
+  }
   return APIC_OK;
 }
 

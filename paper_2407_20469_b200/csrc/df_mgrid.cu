@@ -31,7 +31,7 @@ struct Args {
   DevTables t;
   const DarkDev* leds;
   int n_leds;
-  const float* d_int;
+  ImgSrc src;
   float2* O;               // [chunk][N*N] object spectrum, extended in place
   const float* coef;       // [chunk][nz]
   float2* T;               // [chunk][N*N] N-grid scratch (right-hand side only)
@@ -354,7 +354,7 @@ __device__ __noinline__ void ph_build_p_rows_m(const Args& a, const Ctx& c, int 
 __device__ __noinline__ void ph_cols_rhs_n(const Args& a, const Ctx& c, int slot, int tile, unsigned g, unsigned G) {
   const DarkDev& L = *c.Lp();
   const int line = int(threadIdx.x) & 15, tt = int(threadIdx.x) >> 4;
-  const float* img0 = a.d_int + (size_t(tile) * a.t.n_img + a.t.nb + L.led) * (N * N);
+  const size_t ii = size_t(tile) * a.t.n_img + a.t.nb + L.led;
   __syncthreads();
   for (int st = g; st < N / 16; st += G) {
     const int x = st * 16 + line;
@@ -365,7 +365,7 @@ __device__ __noinline__ void ph_cols_rhs_n(const Args& a, const Ctx& c, int slot
     for (int r = 0; r < 16; ++r) {
       const int fy = tt + 16 * r, ky = fy < N / 2 ? fy : fy - N;
       v[r] = unsigned(ky - L.d_row0) < unsigned(L.d_nrow) ? __ldcg(&tc[fy * N]) : make_float2(0.f, 0.f);
-      im[r] = __ldg(&img0[fy * N + x]);
+      im[r] = img_load(a.src, ii, N * N, fy * N + x);
     }
     fft_regs<N, true, true>(v, c.bufA() + line * S256::LS, tt, c.tw256());
 #pragma unroll
@@ -610,22 +610,18 @@ __global__ void __launch_bounds__(mg::TH, 2) df_mgrid_kernel(const __grid_consta
 }
 
 void launch_darkfield_mgrid(const DevTables& t, const DarkDev* d_leds, int n_leds, const Workspace& w, const LaunchCtx& c,
-                            const float* d_int, int df_iters, float df_tol, int team_size) {
+                            const ImgSrc& src, int df_iters, float df_tol, int team_size) {
   using namespace mg;
   if (n_leds <= 0) return;
   const size_t smem = (size_t(kSmFixed) + 3 * size_t(w.max_unknown)) * sizeof(float2);
-  static bool attr = false;
-  static int sms = 148;
-  if (!attr) {
+  const int sms = c.pd->sms;
+  if (!c.pd->attr_mgrid) {
     cudaFuncSetAttribute(df_mgrid_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 4096);
     cudaFuncSetAttribute(df_mgrid_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    attr = true;
+    c.pd->attr_mgrid = true;
   }
   Args a{};
-  a.t = t; a.leds = d_leds; a.n_leds = n_leds; a.d_int = d_int; a.O = w.O; a.coef = w.coef; a.T = w.T; a.TM = w.TM;
+  a.t = t; a.leds = d_leds; a.n_leds = n_leds; a.src = src; a.O = w.O; a.coef = w.coef; a.T = w.T; a.TM = w.TM;
   a.PF = w.PF; a.vec_w = w.vec_w; a.cg_iters = w.cg_iters; a.max_unknown = w.max_unknown; a.max_iters = df_iters;
   a.tol2 = df_tol * df_tol; a.live = c.live; a.live_count = c.live_count; a.chunk0 = c.chunk0;
   a.n_tiles = c.chunk_tiles; a.work = w.df_work;
@@ -658,7 +654,7 @@ void launch_darkfield_mgrid(const DevTables& t, const DarkDev* d_leds, int n_led
     max_clusters = std::max(1, sms / G - (G > 2 ? 2 : 0));
   const int teams = std::max(1, std::min(max_clusters, c.chunk_tiles));
   cfg.gridDim = dim3(unsigned(G) * unsigned(teams));
-  ProfScope ps(c, CAT_DF_PERSISTENT);
+  ProfScope ps(c, CAT_DF_MGRID);
   cudaLaunchKernelEx(&cfg, df_mgrid_kernel, a);
 }
 

@@ -35,7 +35,7 @@ struct TeamArgs {
   DevTables t;
   const DarkDev* leds;     // device array, processing order
   int n_leds;
-  const float* d_int;
+  ImgSrc src;
   float2* O;               // [chunk][N*N] object spectrum, extended in place
   const float* coef;       // [chunk][nz]
   float2* T;               // [chunk][N*N] transform scratch
@@ -186,7 +186,7 @@ __device__ __noinline__ void phase_cols_p(const TeamArgs& a, const Ctx<N>& c, in
   const DarkDev& L = *c.L;
   const int line = TT<N, true>::line(), tt = TT<N, true>::t();
   constexpr int n_st = N / S::LINES;
-  const float* img0 = a.d_int + (size_t(tile) * a.t.n_img + a.t.nb + L.led) * (N * N);
+  const size_t ii = size_t(tile) * a.t.n_img + a.t.nb + L.led;
   for (int st = g; st < n_st; st += G) {
     const int x = st * S::LINES + line;
     float2* tc = a.T + size_t(slot) * (N * N) + x;
@@ -194,7 +194,7 @@ __device__ __noinline__ void phase_cols_p(const TeamArgs& a, const Ctx<N>& c, in
     float im[S::R];
     load_col_strip<N>(v, tc, tt, L.d_row0, L.d_nrow);
 #pragma unroll
-    for (int r = 0; r < S::R; ++r) im[r] = __ldg(&img0[(tt + S::TPL * r) * N + x]);
+    for (int r = 0; r < S::R; ++r) im[r] = img_load(a.src, ii, N * N, (tt + S::TPL * r) * N + x);
     fft_regs<N, true, true>(v, c.sm + line * S::LS, tt, c.tw);
     float2* pf = a.PF + size_t(slot) * (N * N) + x;
 #pragma unroll
@@ -481,22 +481,18 @@ __global__ void __launch_bounds__(Strip<N, TeamCfg<N>::LINES>::THREADS, TeamCfg<
 
 template <int N>
 static void darkfield_team_n(const DevTables& t, const DarkDev* d_leds, int n_leds, const Workspace& w,
-                             const LaunchCtx& c, const float* d_int, int df_iters, float df_tol, int team_size) {
+                             const LaunchCtx& c, const ImgSrc& src, int df_iters, float df_tol, int team_size) {
   using S = Strip<N, TeamCfg<N>::LINES>;
   const size_t smem = (size_t(S::LINES) * S::LS + S::TW_ENTRIES + 4 * size_t(w.max_unknown)) * sizeof(float2);
-  static bool attr = false;
-  static int sms = 148;
+  const int sms = c.pd->sms;
   int per_sm = 1;
-  if (!attr) {
+  if (!c.pd->attr_team) {
     cudaFuncSetAttribute(df_team_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 4096);
     cudaFuncSetAttribute(df_team_kernel<N>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    attr = true;
+    c.pd->attr_team = true;
   }
   TeamArgs a{};
-  a.t = t; a.leds = d_leds; a.n_leds = n_leds; a.d_int = d_int; a.O = w.O; a.coef = w.coef; a.T = w.T; a.PF = w.PF;
+  a.t = t; a.leds = d_leds; a.n_leds = n_leds; a.src = src; a.O = w.O; a.coef = w.coef; a.T = w.T; a.PF = w.PF;
   a.vec_w = w.vec_w; a.cg_iters = w.cg_iters; a.max_unknown = w.max_unknown; a.max_iters = df_iters;
   a.tol2 = df_tol * df_tol; a.live = c.live; a.live_count = c.live_count; a.chunk0 = c.chunk0;
   a.n_tiles = c.chunk_tiles; a.work = w.df_work;
@@ -524,18 +520,18 @@ static void darkfield_team_n(const DevTables& t, const DarkDev* d_leds, int n_le
     max_clusters = std::max(1, sms / G - (G > 2 ? 2 : 0));
   const int teams = std::max(1, std::min(max_clusters, c.chunk_tiles));
   cfg.gridDim = dim3(unsigned(G) * unsigned(teams));
-  ProfScope ps(c, CAT_DF_PERSISTENT);
+  ProfScope ps(c, CAT_DF_TEAM);
   cudaLaunchKernelEx(&cfg, df_team_kernel<N>, a);
 }
 
 void launch_darkfield_team(const DevTables& t, const DarkDev* d_leds, int n_leds, const Workspace& w, const LaunchCtx& c,
-                           const float* d_int, int df_iters, float df_tol, int team_size) {
+                           const ImgSrc& src, int df_iters, float df_tol, int team_size) {
   if (n_leds <= 0) return;
   switch (t.n) {
-    case 64: darkfield_team_n<64>(t, d_leds, n_leds, w, c, d_int, df_iters, df_tol, team_size); break;
-    case 128: darkfield_team_n<128>(t, d_leds, n_leds, w, c, d_int, df_iters, df_tol, team_size); break;
-    case 256: darkfield_team_n<256>(t, d_leds, n_leds, w, c, d_int, df_iters, df_tol, team_size); break;
-    case 512: darkfield_team_n<512>(t, d_leds, n_leds, w, c, d_int, df_iters, df_tol, team_size); break;
+    case 64: darkfield_team_n<64>(t, d_leds, n_leds, w, c, src, df_iters, df_tol, team_size); break;
+    case 128: darkfield_team_n<128>(t, d_leds, n_leds, w, c, src, df_iters, df_tol, team_size); break;
+    case 256: darkfield_team_n<256>(t, d_leds, n_leds, w, c, src, df_iters, df_tol, team_size); break;
+    case 512: darkfield_team_n<512>(t, d_leds, n_leds, w, c, src, df_iters, df_tol, team_size); break;
   }
 }
 

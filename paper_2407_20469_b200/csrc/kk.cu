@@ -14,18 +14,34 @@
 namespace apic {
 
 // ---------------------------------------------------------------------------------- S0 statistics
-// one CTA per (image, tile): sum, sum of squares and non-finite count of the image
-__global__ void __launch_bounds__(256) image_stats_kernel(const float* __restrict__ d_int, int npix, int n_img,
-                                                          double* __restrict__ stats) {
+// one CTA per (image, tile): sum, sum of squares and non-finite count of the image.  Thread i takes pixels
+// 4 i .. 4 i + 3 (+ 1024 k) in both input forms, with the same association, so that the statistics of the
+// uint16 entry equal those of the fp32 entry on float(count) * scale bit for bit.
+template <bool U16>
+__global__ void __launch_bounds__(256) image_stats_kernel(ImgSrc src, int npix, int n_img, double* __restrict__ stats) {
   const int img = blockIdx.x, tile = blockIdx.y;
-  const float4* p = reinterpret_cast<const float4*>(d_int + (size_t(tile) * n_img + img) * npix);
+  const size_t ii = size_t(tile) * n_img + img;
   float s = 0.f, q = 0.f;
   int bad = 0;
-  for (int i = threadIdx.x; i < npix / 4; i += 256) {
-    float4 v = __ldg(&p[i]);
-    bad += !isfinite(v.x) + !isfinite(v.y) + !isfinite(v.z) + !isfinite(v.w);
-    s += (v.x + v.y) + (v.z + v.w);
-    q += (v.x * v.x + v.y * v.y) + (v.z * v.z + v.w * v.w);
+  if (U16) {
+    const uint2* p = reinterpret_cast<const uint2*>(src.u16 + ii * npix);      // 4 pixels
+    const float sc = src.scale[ii];
+    for (int i = threadIdx.x; i < npix / 4; i += 256) {
+      const uint2 r = __ldg(&p[i]);
+      float4 v;
+      v.x = float(r.x & 0xffffu) * sc; v.y = float(r.x >> 16) * sc; v.z = float(r.y & 0xffffu) * sc; v.w = float(r.y >> 16) * sc;
+      s += (v.x + v.y) + (v.z + v.w);
+      q += (v.x * v.x + v.y * v.y) + (v.z * v.z + v.w * v.w);
+    }
+    bad = (!isfinite(sc) && threadIdx.x == 0) ? 1 : 0;                         // counts are finite; a non-finite scale is bad input
+  } else {
+    const float4* p = reinterpret_cast<const float4*>(src.f32 + ii * npix);
+    for (int i = threadIdx.x; i < npix / 4; i += 256) {
+      float4 v = __ldg(&p[i]);
+      bad += !isfinite(v.x) + !isfinite(v.y) + !isfinite(v.z) + !isfinite(v.w);
+      s += (v.x + v.y) + (v.z + v.w);
+      q += (v.x * v.x + v.y * v.y) + (v.z * v.z + v.w * v.w);
+    }
   }
   __shared__ double sh[3][256];
   sh[0][threadIdx.x] = s;
@@ -40,59 +56,14 @@ __global__ void __launch_bounds__(256) image_stats_kernel(const float* __restric
     }
     __syncthreads();
   }
-  if (threadIdx.x < 3) stats[(size_t(tile) * n_img + img) * 3 + threadIdx.x] = sh[threadIdx.x][0];
+  if (threadIdx.x < 3) stats[ii * 3 + threadIdx.x] = sh[threadIdx.x][0];
 }
 
-void launch_image_stats(const DevTables& t, const float* d_int, int batch, double* stats, const LaunchCtx& c) {
+void launch_image_stats(const DevTables& t, const ImgSrc& src, int batch, double* stats, const LaunchCtx& c) {
   dim3 grid(t.n_img, batch);
   ProfScope ps(c, CAT_STATS);
-  image_stats_kernel<<<grid, 256, 0, c.stream>>>(d_int, t.n * t.n, t.n_img, stats);
-}
-
-// uint16 entry (apic_reconstruct_u16): the statistics pass also converts count * scale into the fp32 working copy
-__global__ void __launch_bounds__(256) image_stats_u16_kernel(const uint16_t* __restrict__ d_raw, const float* __restrict__ d_scale,
-                                                              float* __restrict__ d_out, int npix, int n_img,
-                                                              double* __restrict__ stats) {
-  const int img = blockIdx.x, tile = blockIdx.y;
-  const size_t off = (size_t(tile) * n_img + img) * npix;
-  const uint4* p = reinterpret_cast<const uint4*>(d_raw + off);          // 8 pixels
-  float4* o = reinterpret_cast<float4*>(d_out + off);
-  const float sc = d_scale[size_t(tile) * n_img + img];
-  float s = 0.f, q = 0.f;
-  for (int i = threadIdx.x; i < npix / 8; i += 256) {
-    const uint4 r = __ldg(&p[i]);
-    float4 a, b;
-    a.x = float(r.x & 0xffffu) * sc; a.y = float(r.x >> 16) * sc; a.z = float(r.y & 0xffffu) * sc; a.w = float(r.y >> 16) * sc;
-    b.x = float(r.z & 0xffffu) * sc; b.y = float(r.z >> 16) * sc; b.z = float(r.w & 0xffffu) * sc; b.w = float(r.w >> 16) * sc;
-    o[2 * i] = a;
-    o[2 * i + 1] = b;
-    // same association as image_stats_kernel, so that the statistics equal those of the fp32 entry on the same values
-    s += (a.x + a.y) + (a.z + a.w);
-    q += (a.x * a.x + a.y * a.y) + (a.z * a.z + a.w * a.w);
-    s += (b.x + b.y) + (b.z + b.w);
-    q += (b.x * b.x + b.y * b.y) + (b.z * b.z + b.w * b.w);
-  }
-  __shared__ double sh[3][256];
-  sh[0][threadIdx.x] = s;
-  sh[1][threadIdx.x] = q;
-  sh[2][threadIdx.x] = isfinite(sc) ? 0.0 : double(threadIdx.x == 0);      // counts are finite; a non-finite scale is bad input
-  __syncthreads();
-  for (int o2 = 128; o2 > 0; o2 >>= 1) {
-    if (threadIdx.x < o2) {
-      sh[0][threadIdx.x] += sh[0][threadIdx.x + o2];
-      sh[1][threadIdx.x] += sh[1][threadIdx.x + o2];
-      sh[2][threadIdx.x] += sh[2][threadIdx.x + o2];
-    }
-    __syncthreads();
-  }
-  if (threadIdx.x < 3) stats[(size_t(tile) * n_img + img) * 3 + threadIdx.x] = sh[threadIdx.x][0];
-}
-
-void launch_image_stats_u16(const DevTables& t, const uint16_t* d_raw, const float* d_scale, float* d_out, int batch,
-                            double* stats, const LaunchCtx& c) {
-  dim3 grid(t.n_img, batch);
-  ProfScope ps(c, CAT_STATS);
-  image_stats_u16_kernel<<<grid, 256, 0, c.stream>>>(d_raw, d_scale, d_out, t.n * t.n, t.n_img, stats);
+  if (src.u16) image_stats_kernel<true><<<grid, 256, 0, c.stream>>>(src, t.n * t.n, t.n_img, stats);
+  else image_stats_kernel<false><<<grid, 256, 0, c.stream>>>(src, t.n * t.n, t.n_img, stats);
 }
 
 // one warp: per-tile status (O1, BASELINE.json item 5, R18) and the ordered list of
@@ -160,7 +131,7 @@ void launch_zero_dead(const DevTables& t, const int32_t* status, int batch, floa
 // ---------------------------------------------------------------------------------- S1-S2
 template <int N>
 __global__ void __launch_bounds__(Strip<N>::THREADS, Strip<N>::MINB)
-kk_log_rowfft(DevTables t, const float* __restrict__ d_int, const double* __restrict__ stats, float floor_rel,
+kk_log_rowfft(DevTables t, ImgSrc src, const double* __restrict__ stats, float floor_rel,
               float2* __restrict__ G, const int32_t* __restrict__ live, const int32_t* __restrict__ live_count,
               int chunk0) {
   using S = Strip<N>;
@@ -170,12 +141,12 @@ kk_log_rowfft(DevTables t, const float* __restrict__ d_int, const double* __rest
   const int tile = resolve_tile_idx(live, live_count, chunk0, slot);
   if (tile < 0) return;
   const int line = TH::line(), tt = TH::t(), y = blockIdx.x * S::LINES + line;
-  const float* img = d_int + (size_t(tile) * t.n_img + led) * (N * N) + y * N;
+  const size_t ii = size_t(tile) * t.n_img + led;
   const float mean = float(stats[(size_t(tile) * t.n_img + led) * 3] / double(N * N));
   const float lo = floor_rel * mean;                                   // R6
   float2 v[S::R];
 #pragma unroll
-  for (int r = 0; r < S::R; ++r) v[r] = make_float2(logf(fmaxf(__ldg(&img[tt + S::TPL * r]), lo)), 0.f);  // Re of Eq. 4
+  for (int r = 0; r < S::R; ++r) v[r] = make_float2(logf(fmaxf(img_load(src, ii, N * N, y * N + tt + S::TPL * r), lo)), 0.f);  // Re of Eq. 4
   fft_regs<N, false>(v, sm + line * S::LS, tt, t.tw);
   float2* g = G + (size_t(slot) * t.nb + led) * (N * N) + y * N;
 #pragma unroll
@@ -265,22 +236,21 @@ kk_col_gather(DevTables t, const float2* __restrict__ G, float2* __restrict__ Sp
 }
 
 template <int N>
-static void launch_kk_n(const DevTables& t, const Workspace& w, const LaunchCtx& c, const float* d_int,
+static void launch_kk_n(const DevTables& t, const Workspace& w, const LaunchCtx& c, const ImgSrc& src,
                         const double* stats, float floor_rel) {
   using S = Strip<N>;
   constexpr int TH = S::THREADS;
   constexpr size_t SM = S::SMEM;
-  static bool attr = false;
-  if (!attr) {
+  if (!c.pd->attr_kk) {
     cudaFuncSetAttribute(kk_log_rowfft<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
     cudaFuncSetAttribute(kk_col_mask<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
     cudaFuncSetAttribute(kk_row_exp<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
     cudaFuncSetAttribute(kk_col_gather<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
-    attr = true;
+    c.pd->attr_kk = true;
   }
   dim3 grid(N / S::LINES, t.nb, c.chunk_tiles);
   { ProfScope ps(c, CAT_KK_LOG_ROWFFT);
-    kk_log_rowfft<N><<<grid, TH, SM, c.stream>>>(t, d_int, stats, floor_rel, w.G, c.live, c.live_count, c.chunk0); }
+    kk_log_rowfft<N><<<grid, TH, SM, c.stream>>>(t, src, stats, floor_rel, w.G, c.live, c.live_count, c.chunk0); }
   { ProfScope ps(c, CAT_KK_COL_MASK);
     kk_col_mask<N><<<grid, TH, SM, c.stream>>>(t, w.G, c.live_count, c.chunk0); }
   { ProfScope ps(c, CAT_KK_ROW_EXP);
@@ -290,13 +260,13 @@ static void launch_kk_n(const DevTables& t, const Workspace& w, const LaunchCtx&
     kk_col_gather<N><<<grid4, TH, SM, c.stream>>>(t, w.G, w.S, c.live_count, c.chunk0); }
 }
 
-void launch_kk(const DevTables& t, const Workspace& w, const LaunchCtx& c, const float* d_int, const double* stats,
+void launch_kk(const DevTables& t, const Workspace& w, const LaunchCtx& c, const ImgSrc& src, const double* stats,
                float floor_rel) {
   switch (t.n) {
-    case 64: launch_kk_n<64>(t, w, c, d_int, stats, floor_rel); break;
-    case 128: launch_kk_n<128>(t, w, c, d_int, stats, floor_rel); break;
-    case 256: launch_kk_n<256>(t, w, c, d_int, stats, floor_rel); break;
-    case 512: launch_kk_n<512>(t, w, c, d_int, stats, floor_rel); break;
+    case 64: launch_kk_n<64>(t, w, c, src, stats, floor_rel); break;
+    case 128: launch_kk_n<128>(t, w, c, src, stats, floor_rel); break;
+    case 256: launch_kk_n<256>(t, w, c, src, stats, floor_rel); break;
+    case 512: launch_kk_n<512>(t, w, c, src, stats, floor_rel); break;
   }
 }
 

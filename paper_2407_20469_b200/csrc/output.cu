@@ -92,11 +92,10 @@ static void output_n(const DevTables& t, const Workspace& w, const LaunchCtx& c,
   using S = Strip<N>;
   constexpr int TH = S::THREADS, kLines = S::LINES;
   constexpr size_t SM = S::SMEM;
-  static bool attr = false;
-  if (!attr) {
+  if (!c.pd->attr_out) {
     cudaFuncSetAttribute(out_rows<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
     cudaFuncSetAttribute(out_cols<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
-    attr = true;
+    c.pd->attr_out = true;
   }
   dim3 g1((t.known_nrow + kLines - 1) / kLines, t.u, c.chunk_tiles);
   { ProfScope ps(c, CAT_OUT_ROWS);

@@ -72,20 +72,23 @@ struct Workspace {
   float2* T;               // [chunk][N*N] transform scratch
   float2* PF;              // [chunk][N*N] p = F^-1 P_hat of the current darkfield LED
   float2* TM;              // [chunk][N*N] transform scratch on the reduced grid (df_mgrid.cu)
-  float2* vec_d;           // [chunk][max_eq]
-  float2* vec_x;           // [chunk][max_unknown]
-  float2* vec_s;
-  float2* vec_p;
-  float2* vec_w;
-  float* dot_part;         // [chunk][dot_parts]
-  int dot_parts;
-  float* cg_scal;          // [chunk][4]: gamma, gamma0, -, -
-  int32_t* cg_done;        // [chunk]
+  float2* vec_w;           // [chunk][max_unknown] w = C^H M_Q C pdir of the current CG iteration
+  float2* vec_x;           // [chunk][max_unknown] CG iterate
+  float2* vec_s;           // [chunk][max_unknown] CG residual of the normal equations
   int32_t* cg_iters;       // [chunk][n_dark_used]
-  int32_t* df_sync;        // [2 + chunk] persistent scheduler: ticket, finished tiles, per-tile progress
   unsigned long long* df_work;   // [1] nominal flop (5 L log2 L per L-point line transform) executed by the darkfield kernels
   float2* TOUT;            // [chunk][N][uN]
   int max_eq, max_unknown;
+};
+
+// Where a step's intensities come from: fp32 values in radiometric units (apic_reconstruct) or raw uint16
+// camera counts with one factor per image (apic_reconstruct_u16; PAPER.md:199 - exposures differ between
+// NA-matching and darkfield frames).  The conversion count * scale happens in the load itself, in fp32, so both
+// entries see the same bits for the same values and no fp32 working copy of the counts exists.
+struct ImgSrc {
+  const float* f32;        // [batch][n_img][N*N] or nullptr
+  const uint16_t* u16;     // [batch][n_img][N*N] or nullptr
+  const float* scale;      // [batch][n_img] (uint16 form only)
 };
 
 // Batch-level state
@@ -98,9 +101,16 @@ struct BatchState {
 // ------------------------------------------------------------------ per-kernel timing (apic_profile_*)
 enum KernelCat {
   CAT_STATS = 0, CAT_KK_LOG_ROWFFT, CAT_KK_COL_MASK, CAT_KK_ROW_EXP, CAT_KK_COL_GATHER, CAT_AB_PRODUCTS, CAT_AB_GRAM,
-  CAT_AB_SOLVE, CAT_STITCH, CAT_DF_BUILD_P_ROWS, CAT_DF_COLS_P, CAT_DF_ROWS_RHS, CAT_DF_ROWS_Q, CAT_DF_COLS_MUL,
-  CAT_DF_ROWS_U_SCATTER, CAT_DF_ROWS_U_GATHER, CAT_DF_CG_VECTOR, CAT_DF_EXTEND, CAT_OUT_ROWS, CAT_OUT_COLS,
-  CAT_PUPIL, CAT_DF_PERSISTENT, CAT_COUNT
+  CAT_AB_SOLVE, CAT_STITCH, CAT_OUT_ROWS, CAT_OUT_COLS, CAT_PUPIL, CAT_DF_MGRID, CAT_DF_TEAM, CAT_COUNT
+};
+
+// Per-plan record of what has been set up on the plan's device (function attributes are per device, so the
+// flags live in the plan, not in process-wide statics: a second plan on another GPU does its own set-up).
+struct PlanDevice {
+  int device = 0;          // CUDA device the plan was created on (apic_reconstruct runs there)
+  int sms = 0;             // its SM count
+  int l2_bytes = 0;        // its L2 size
+  bool attr_kk = false, attr_ab = false, attr_out = false, attr_team = false, attr_mgrid = false;
 };
 
 struct Profiler {
@@ -121,6 +131,7 @@ struct LaunchCtx {
   const int32_t* live_count;
   int chunk0;              // first live-list position of this chunk
   int chunk_tiles;         // grid size in tiles (CTAs beyond live_count exit)
+  PlanDevice* pd;          // per-plan device state (attribute set-up flags, SM count)
 };
 
 // stats / status (batch-level)
@@ -143,31 +154,25 @@ struct ProfScope {
   }
 };
 
-void launch_image_stats(const DevTables& t, const float* d_int, int batch, double* stats, const LaunchCtx& c);
-// the same pass over uint16 counts: converts (count * scale[tile][image]) into d_out (fp32, same layout) on the way
-void launch_image_stats_u16(const DevTables& t, const uint16_t* d_raw, const float* d_scale, float* d_out, int batch,
-                            double* stats, const LaunchCtx& c);
+void launch_image_stats(const DevTables& t, const ImgSrc& src, int batch, double* stats, const LaunchCtx& c);
 void launch_tile_status(const DevTables& t, const double* stats, int batch, int bg_mode, float bg_thr,
                         int32_t* status, int32_t* live, int32_t* live_count, const LaunchCtx& c);
 void launch_zero_dead(const DevTables& t, const int32_t* status, int batch, float* field, float* zern,
                       float* pupil, const LaunchCtx& c);
 
 // KK (S1-S5)
-void launch_kk(const DevTables& t, const Workspace& w, const LaunchCtx& c, const float* d_int,
+void launch_kk(const DevTables& t, const Workspace& w, const LaunchCtx& c, const ImgSrc& src,
                const double* stats, float floor_rel);
 // aberration (S6) + stitching (S7)
 void launch_aberration(const DevTables& t, const Workspace& w, const LaunchCtx& c, int refine_iters,
                        float* d_zernike, int32_t* d_status);
 void launch_stitch(const DevTables& t, const Workspace& w, const LaunchCtx& c);
-// darkfield (S8-S10) for one LED
-void launch_darkfield_led(const DevTables& t, const DarkDev& L, int led_pos, int n_dark_used, const Workspace& w,
-                          const LaunchCtx& c, const float* d_int, int df_iters, float df_tol, int df_mode);
 // darkfield (S8-S10), every LED in one launch (df_team.cu)
 void launch_darkfield_team(const DevTables& t, const DarkDev* d_leds, int n_leds, const Workspace& w, const LaunchCtx& c,
-                           const float* d_int, int df_iters, float df_tol, int team_size);
+                           const ImgSrc& src, int df_iters, float df_tol, int team_size);
 // darkfield (S8-S10) on reduced cyclic grids, every LED in one launch (df_mgrid.cu; N = 256)
 void launch_darkfield_mgrid(const DevTables& t, const DarkDev* d_leds, int n_leds, const Workspace& w, const LaunchCtx& c,
-                            const float* d_int, int df_iters, float df_tol, int team_size);
+                            const ImgSrc& src, int df_iters, float df_tol, int team_size);
 int launch_fft2d_xy(float2* d, int mx, int my, int batch, int mode, const float2* tw_xy, cudaStream_t s);
 // outputs
 void launch_output(const DevTables& t, const Workspace& w, const LaunchCtx& c, float* d_field, float* d_pupil);
@@ -176,6 +181,11 @@ void launch_output(const DevTables& t, const Workspace& w, const LaunchCtx& c, f
 int launch_fft2d(float2* d, int n, int batch, bool inverse, const float2* tw, cudaStream_t s);
 
 #ifdef __CUDACC__
+// pixel `px` of image `img` (= tile * n_img + led) of `npix` pixels, in radiometric units
+__device__ __forceinline__ float img_load(const ImgSrc& s, size_t img, int npix, int px) {
+  if (s.u16) return float(__ldg(&s.u16[img * size_t(npix) + px])) * __ldg(&s.scale[img]);
+  return __ldg(&s.f32[img * size_t(npix) + px]);
+}
 // tile handled by chunk-local slot `slot` (-1: beyond the live list)
 __device__ __forceinline__ int resolve_tile_idx(const int32_t* __restrict__ live,
                                                 const int32_t* __restrict__ live_count, int chunk0, int slot) {

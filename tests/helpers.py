@@ -17,6 +17,12 @@ def oracle_params(cfg, **kw) -> O.OracleParams:
                           noll=list(cfg.noll_fit), **kw)
 
 
+def plan_from_config(A, cfg, **opts):
+    """apic_plan for an apic_synth config (optics, LED layout and fitted Noll terms of the recipe)."""
+    from apic_synth import plan_args
+    return A.Plan(*plan_args(cfg), **opts)
+
+
 def truth_object_spectrum(cfg, truth, radius):
     """What the reconstruction must equal inside the synthetic band:
     O_true(k) * exp(j*tilt(k)) * exp(-j*arg O_true(0)), centred [N][N]; a pupil tilt (Noll 2, 3)

@@ -11,7 +11,7 @@ import numpy as np
 import pytest
 
 from apic_synth import get_config, led_kvectors
-from helpers import read_golden_table
+from helpers import plan_from_config, read_golden_table
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
@@ -124,7 +124,7 @@ def test_no_cpu_fallback(A):
         pytest.skip("a CUDA device is present")
     cfg = get_config(0)
     with pytest.raises(A.ApicError, match="CUDA"):
-        A.Plan.from_config(cfg)
+        plan_from_config(A, cfg)
 
 
 @pytest.mark.parametrize("index,tile_n", [(2, 256), (3, 256), (2, 64)])
