@@ -90,7 +90,10 @@ typedef struct {
                             cluster barriers between phases); at N = 256 it runs the CG mat-vecs
                             on per-LED reduced cyclic grids.  3 = the team
                             kernel on the full N x N grid (what other N run; kept at N = 256 as a
-                            cross-check of the reduced grids)                                   */
+                            cross-check of the reduced grids).  4 = the reduced-grid solver with
+                            strips staged into shared memory by the async proxy (cp.async.bulk +
+                            mbarrier, strip-major scratch) and the CG vectors distributed over the
+                            team (N = 256; other N fall back to the full-grid team kernel)      */
   int df_team;           /* CTAs per tile, 1..8; 0 = chosen from the pass size (as many as the
                             pass leaves resident CTA slots for)                                 */
 } apic_params;

@@ -318,6 +318,11 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
     ok = ok && plan->upload(&q.dmap, L.dmap);
     ok = ok && plan->upload(&q.qmap, L.qmap);
     q.mx = L.mx; q.my = L.my;
+    for (int st = 0; st <= kMaxUStrips; ++st)
+      q.u_strip_off[st] = L.u_row_off[size_t(std::min(16 * st, L.u_nrow))];
+    if ((L.u_nrow + 15) / 16 > kMaxUStrips) ok = false;
+    auto modp = [](int k, int m) { return ((k % m) + m) % m; };
+    q.u0m = modp(L.u_row0, L.my); q.q0m = modp(L.q_row0, L.my); q.d0m = modp(L.d_row0, L.my);
     ok = ok && plan->upload(&q.dmap_m, L.dmap_m);
     ok = ok && plan->upload(&q.qmask_m, L.qmask_m);
     plan->dark.push_back(q);
@@ -328,7 +333,7 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
   const size_t nn = size_t(n) * n;
   int chunk = p->chunk_tiles;
   if (chunk <= 0) {
-    if (n == 256 && p->df_mode == 0 && !h.dark.empty()) {
+    if (n == 256 && (p->df_mode == 0 || p->df_mode == 4) && !h.dark.empty()) {
       // reduced-grid darkfield kernel: its CG working set is ~0.3 MB per tile (TM + p_M on grids of 15-20 k bins),
       // so the pass is sized for the kernel's scheduler instead: up to two tiles per SM (one CTA per tile)
       chunk = 2 * std::max(1, plan->pd.sms);
@@ -411,6 +416,8 @@ static int reconstruct_impl(apic_plan* plan, int zi, const ImgSrc& src, int batc
     launch_stitch(t, w, c);                                                                   // S7
     if (p.df_mode == 0 && t.n == 256)                                                         // S8-S10
       launch_darkfield_mgrid(t, plan->d_dark, n_dark_used, w, c, src, p.df_iters, p.df_tol, p.df_team);
+    else if (p.df_mode == 4 && t.n == 256)
+      launch_darkfield_tma(t, plan->d_dark, plan->dark.data(), n_dark_used, w, c, src, p.df_iters, p.df_tol, p.df_team);
     else
       launch_darkfield_team(t, plan->d_dark, n_dark_used, w, c, src, p.df_iters, p.df_tol, p.df_team);
     launch_output(t, w, c, d_field, d_pupil);                                                 // S10
@@ -633,7 +640,7 @@ int apic_last_launch_count(const apic_plan* plan) { return plan ? plan->launches
 
 static const char* kCatNames[CAT_COUNT] = {
     "stats_status", "kk_log_rowfft", "kk_col_mask", "kk_row_exp", "kk_col_gather", "ab_pair_products", "ab_gram",
-    "ab_solve", "stitch", "out_rows", "out_cols", "pupil", "df_mgrid_kernel", "df_team_kernel"};
+    "ab_solve", "stitch", "out_rows", "out_cols", "pupil", "df_mgrid_kernel", "df_team_kernel", "df_tma_kernel"};
 
 int apic_profile_categories(void) { return CAT_COUNT; }
 const char* apic_profile_category_name(int cat) { return (cat >= 0 && cat < CAT_COUNT) ? kCatNames[cat] : ""; }

@@ -123,7 +123,7 @@ bool build_geometry(const apic_params& p, HostTables& t, std::string& err) {
   if (p.df_iters < 1) { err = "df_iters must be >= 1"; return false; }
   if (p.bg_mode < 0 || p.bg_mode > 2) { err = "bg_mode must be 0, 1 or 2"; return false; }
   if (p.max_batch < 1) { err = "max_batch must be >= 1"; return false; }
-  if (p.df_mode != 0 && p.df_mode != 3) { err = "df_mode must be 0 (team kernel; reduced cyclic grids at N = 256) or 3 (team kernel on the full N x N grid)"; return false; }
+  if (p.df_mode != 0 && p.df_mode != 3 && p.df_mode != 4) { err = "df_mode must be 0 (team kernel; reduced cyclic grids at N = 256), 3 (team kernel on the full N x N grid) or 4 (reduced grids with async-proxy staging)"; return false; }
   if (!(p.df_team == 0 || p.df_team == 1 || p.df_team == 2 || p.df_team == 4 || p.df_team == 8)) {
     err = "df_team must be 0 (auto), 1, 2, 4 or 8"; return false;
   }
@@ -336,16 +336,19 @@ bool build_geometry(const apic_params& p, HostTables& t, std::string& err) {
     L.disc_f.resize(nD);
     L.zern.resize(size_t(nD) * nz);
     int eu = 0, ep = nU;
+    L.u_row_off.assign(size_t(L.u_nrow) + 1, 0);
     for (int iy = 0; iy < n; ++iy)
       for (int ix = 0; ix < n; ++ix) {
         size_t q = size_t(iy) * n + ix;
         if (!d.v[q]) continue;
+        if (U.v[q]) ++L.u_row_off[size_t(iy - h - L.u_row0) + 1];
         int e = U.v[q] ? eu++ : ep++;
         ent[q] = e;
         int kx = ix - h, ky = iy - h;
         L.disc_f[e] = fft_index(n, kx, ky);
         for (int a = 0; a < nz; ++a) L.zern[size_t(e) * nz + a] = float(zern_at(t.noll[a], kx, ky, kap));
       }
+    for (int r = 0; r < L.u_nrow; ++r) L.u_row_off[size_t(r) + 1] += L.u_row_off[size_t(r)];
     L.dmap.assign(size_t(n) * L.d_ncol, -1);
     for (int iy = 0; iy < n; ++iy)
       for (int c = 0; c < L.d_ncol; ++c) {

@@ -27,6 +27,7 @@ struct DarkLed {
   int q_col0 = 0, q_ncol = 0;  // bbox of Q
   int q_row0 = 0, q_nrow = 0;
   std::vector<int32_t> disc_f; // [n_disc] FFT-order linear index of each disc entry
+  std::vector<int32_t> u_row_off; // [u_nrow+1] first U entry of each row of the U bbox (U entries are row-major)
   std::vector<float> zern;     // [n_disc][nz] Z_j(K + kappa)
   std::vector<int32_t> dmap;   // [N (fy)][d_ncol] -> disc entry or -1
   std::vector<int32_t> qmap;   // [N (fy)][q_ncol] -> equation index or -1

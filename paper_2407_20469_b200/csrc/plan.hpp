@@ -41,6 +41,8 @@ struct DevTables {
   const float* pupil_zern;       // [n_pupil][nz]
 };
 
+constexpr int kMaxUStrips = 16;            // a disc spans <= 2R + 1 <= 0.34 N rows: <= 11 strips of 16 rows at N = 512
+
 struct DarkDev {
   int n_unknown, n_disc, n_eq;
   int d_col0, d_ncol, d_row0, d_nrow;   // disc bbox (centred)
@@ -54,6 +56,8 @@ struct DarkDev {
   int mx, my;                           // reduced cyclic grid of the CG mat-vecs (geometry.hpp)
   const int32_t* dmap_m;                // [my][mx] -> disc entry | -1
   const uint8_t* qmask_m;               // [my][mx] -> 1 on Q
+  int u_strip_off[kMaxUStrips + 1];     // first U entry of each 16-row strip of the U rows (U entries are row-major)
+  int u0m, q0m, d0m;                    // u_row0, q_row0, d_row0 mod my (first physical row on the reduced grid)
 };
 
 constexpr int kGramRows = 512;          // rows per Gram partial (aberration kernels)
@@ -101,7 +105,7 @@ struct BatchState {
 // ------------------------------------------------------------------ per-kernel timing (apic_profile_*)
 enum KernelCat {
   CAT_STATS = 0, CAT_KK_LOG_ROWFFT, CAT_KK_COL_MASK, CAT_KK_ROW_EXP, CAT_KK_COL_GATHER, CAT_AB_PRODUCTS, CAT_AB_GRAM,
-  CAT_AB_SOLVE, CAT_STITCH, CAT_OUT_ROWS, CAT_OUT_COLS, CAT_PUPIL, CAT_DF_MGRID, CAT_DF_TEAM, CAT_COUNT
+  CAT_AB_SOLVE, CAT_STITCH, CAT_OUT_ROWS, CAT_OUT_COLS, CAT_PUPIL, CAT_DF_MGRID, CAT_DF_TEAM, CAT_DF_TMA, CAT_COUNT
 };
 
 // Per-plan record of what has been set up on the plan's device (function attributes are per device, so the
@@ -110,7 +114,7 @@ struct PlanDevice {
   int device = 0;          // CUDA device the plan was created on (apic_reconstruct runs there)
   int sms = 0;             // its SM count
   int l2_bytes = 0;        // its L2 size
-  bool attr_kk = false, attr_ab = false, attr_out = false, attr_team = false, attr_mgrid = false;
+  bool attr_kk = false, attr_ab = false, attr_out = false, attr_team = false, attr_mgrid = false, attr_tma = false;
 };
 
 struct Profiler {
@@ -173,6 +177,10 @@ void launch_darkfield_team(const DevTables& t, const DarkDev* d_leds, int n_leds
 // darkfield (S8-S10) on reduced cyclic grids, every LED in one launch (df_mgrid.cu; N = 256)
 void launch_darkfield_mgrid(const DevTables& t, const DarkDev* d_leds, int n_leds, const Workspace& w, const LaunchCtx& c,
                             const ImgSrc& src, int df_iters, float df_tol, int team_size);
+// the same solver with strips staged by the async proxy (cp.async.bulk + mbarrier) and distributed CG vectors
+// (df_tma.cu; N = 256, df_mode 4); h_leds = host copy of d_leds
+void launch_darkfield_tma(const DevTables& t, const DarkDev* d_leds, const DarkDev* h_leds, int n_leds, const Workspace& w,
+                          const LaunchCtx& c, const ImgSrc& src, int df_iters, float df_tol, int team_size);
 int launch_fft2d_xy(float2* d, int mx, int my, int batch, int mode, const float2* tw_xy, cudaStream_t s);
 // outputs
 void launch_output(const DevTables& t, const Workspace& w, const LaunchCtx& c, float* d_field, float* d_pupil);

@@ -237,6 +237,19 @@ def test_config2_full_size_bench_configuration(A):
     sample = [0, 9, 18, 27, 37, 45, 54, 63]
     refs, geo = oracle_reconstruct(cfg, stacks[sample])
     sets = O.darkfield_sets(geo)[0]
+    # df_mode 4: the same reduced-grid solver with strips staged by the async proxy (cp.async.bulk + mbarrier),
+    # strip-major scratch and the CG vectors distributed over the team; whole batch in the bench's launch
+    # configuration, the sampled tiles against the oracle band by band, every tile against df_mode 0
+    plan4, field4, zern4, pupil4, status4 = gpu_reconstruct(A, cfg, stacks, df_mode=4)
+    assert np.all(status4 == 0) and np.array_equal(zern4, zern)
+    og4 = plan4.debug_buffer(A.DBG_OBJECT_SPECTRUM, 64).cpu().numpy().reshape(64, 256, 256)
+    for ref, b in zip(refs, sample):
+        check_tile(ref, field4[b], zern4[b], pupil4[b], status4[b], f"cfg2 tile {b} (df_mode 4)")
+        check_bands(geo, sets, og4[b], ref, f"cfg2 tile {b} (df_mode 4)")
+    for b in tiles:
+        assert rel_l2(field4[b], field[b]) < 2e-5, b
+    _, field4b, _, _, _ = gpu_reconstruct(A, cfg, stacks, df_mode=4)
+    assert np.array_equal(field4, field4b)                              # bit-reproducible
     og = plan.debug_buffer(A.DBG_OBJECT_SPECTRUM, 64).cpu().numpy().reshape(64, 256, 256)
     worst = {}
     for ref, b in zip(refs, sample):
