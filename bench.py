@@ -9,7 +9,8 @@ Poisson noise, 3x output grid) - the batched 256x256 configuration the north-sta
 on (config 1 is a single tile, i.e. a latency case).  Prints ONE JSON line.
 
   value     output megapixels/s with the inputs resident in HBM (CUDA events, max over ranks)
-  e2e       the same metric through apic_reconstruct_host with pinned HOST buffers (H2D + D2H inside)
+  e2e       the same metric through apic_submit_host / apic_wait_host with pinned HOST buffers (H2D + D2H inside;
+            two batches in flight), and through the blocking apic_reconstruct_host beside it
   roofline  the dominant kernel (df_mgrid_kernel: the darkfield CG on reduced cyclic grids), timed live by CUDA
             events inside the library on the launching stream, against fp32 peaks MEASURED in this run
             (apic_measure_peak: FFMA and FADD register loops, shared-memory reads)
@@ -373,46 +374,66 @@ def run_batch(ctx):
     algo_bytes = tiles * (host[0].nbytes + on * on * 8 + n * n * 8 + nz * 4 + 4)
     roofline = roofline_line(ctx, plan, prof, clocks, tiles, workload, ms / args.steps, algo_bytes)
 
-    # ---- end to end through the host-buffer entry point (pinned memory, copies inside the timed region)
+    # ---- end to end through the host-buffer entry points (pinned memory, copies inside the timed region)
     e2e = None
     if not args.no_e2e:
         hx = torch.from_numpy(host).pin_memory()
-        hf = torch.empty((tiles, on, on), dtype=torch.complex64).pin_memory()
-        hz = torch.empty((tiles, nz), dtype=torch.float32).pin_memory()
-        hp = torch.empty((tiles, n, n), dtype=torch.complex64).pin_memory()
-        hs = torch.empty((tiles,), dtype=torch.int32).pin_memory()
+        outs = [(torch.empty((tiles, on, on), dtype=torch.complex64).pin_memory(),
+                 torch.empty((tiles, nz), dtype=torch.float32).pin_memory(),
+                 torch.empty((tiles, n, n), dtype=torch.complex64).pin_memory(),
+                 torch.empty((tiles,), dtype=torch.int32).pin_memory()) for _ in range(2)]
+        hf, hz, hp, hs = outs[0]
         stream = torch.cuda.current_stream().cuda_stream
-        plan.reconstruct_host(hx, hf, hz, hp, hs, stream)          # warm-up (allocates the staging buffers)
-        k2 = max(1, min(args.steps, 5))
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(k2):
-            plan.reconstruct_host(hx, hf, hz, hp, hs, stream)
-        torch.cuda.synchronize()
-        dt = ctx["max_over_ranks"](time.perf_counter() - t0, dist, device="cuda")
-        assert np.array_equal(hf.numpy(), out[0].cpu().numpy()), "host entry and device entry disagree"
-        e2e = {"value": world * k2 * tiles * on * on / 1e6 / dt, "unit": UNIT,
-               "h2d_bytes_per_step": int(hx.numel() * 4),
-               "d2h_bytes_per_step": int(hf.numel() * 8 + hz.numel() * 4 + hp.numel() * 8 + hs.numel() * 4),
-               "steps": k2, "api": "apic_reconstruct_host (pinned host buffers, fp32 intensities)"}
+        k2 = max(6, min(args.steps, 10))
+        ref_field = out[0].cpu().numpy()
+
+        def timed(step_fn, drain_fn=None):
+            """k2 steps after one warm-up step (which allocates the staging buffers); seconds, max over ranks."""
+            step_fn(0)
+            if drain_fn:
+                drain_fn()
+            torch.cuda.synchronize()
+            barrier()
+            t0 = time.perf_counter()
+            for i in range(k2):
+                step_fn(i)
+            if drain_fn:
+                drain_fn()
+            torch.cuda.synchronize()
+            return ctx["max_over_ranks"](time.perf_counter() - t0, dist, device="cuda")
+
+        def drain():
+            plan.wait_host(0)
+            plan.wait_host(1)
+
+        # (1) streaming: apic_submit_host / apic_wait_host, one batch in flight per pipeline slot; every step uploads
+        # its inputs from pinned memory and its results are read back to pinned memory (two output buffer sets)
+        dt = timed(lambda i: plan.submit_host(i & 1, hx, *outs[i & 1]), drain)
+        assert all(np.array_equal(o[0].numpy(), ref_field) for o in outs), "streaming host entry and device entry disagree"
+        d2h = int(hf.numel() * 8 + hz.numel() * 4 + hp.numel() * 8 + hs.numel() * 4)
+        e2e = {"value": world * k2 * tiles * on * on / 1e6 / dt, "unit": UNIT, "h2d_bytes_per_step": int(hx.numel() * 4),
+               "d2h_bytes_per_step": d2h, "steps": k2,
+               "api": "apic_submit_host / apic_wait_host (pinned host buffers, fp32 intensities, two batches in flight)"}
+        # (2) one blocking call per step: upload, kernels and download of a step overlap only inside the call
+        dt = timed(lambda i: plan.reconstruct_host(hx, hf, hz, hp, hs, stream))
+        assert np.array_equal(hf.numpy(), ref_field), "host entry and device entry disagree"
+        e2e["single_call"] = {"value": world * k2 * tiles * on * on / 1e6 / dt, "unit": UNIT,
+                              "api": "apic_reconstruct_host (blocking, sub-batches pipelined inside the call)"}
         if cfg.noise == "poisson":
             # the same step from the camera's uint16 counts (BASELINE.json config 2: "uint16 raw converted to fp32"):
-            # apic_reconstruct_host_u16, half the host-to-device bytes; reported beside the fp32 number, not instead
+            # half the host-to-device bytes; reported beside the fp32 number, not instead
             gains = np.array([[t.gain_bright] * cfg.n_bright + [t.gain_dark] * cfg.n_dark for t in truths])
             gains = np.concatenate([gains] * reps)[:tiles]
             raw = np.rint(host.astype(np.float64) * gains[:, :, None, None]).astype(np.uint16)
             hr = torch.from_numpy(raw).pin_memory()
             hsc = torch.from_numpy((1.0 / gains).astype(np.float32)).pin_memory()
-            plan.reconstruct_host_u16(hr, hsc, hf, hz, hp, hs, stream)
-            barrier()
-            t0 = time.perf_counter()
-            for _ in range(k2):
-                plan.reconstruct_host_u16(hr, hsc, hf, hz, hp, hs, stream)
-            torch.cuda.synchronize()
-            dt = ctx["max_over_ranks"](time.perf_counter() - t0, dist, device="cuda")
+            dt = timed(lambda i: plan.submit_host_u16(i & 1, hr, hsc, *outs[i & 1]), drain)
             e2e["u16"] = {"value": world * k2 * tiles * on * on / 1e6 / dt, "unit": UNIT,
-                          "h2d_bytes_per_step": int(hr.numel() * 2 + hsc.numel() * 4),
-                          "api": "apic_reconstruct_host_u16 (pinned host buffers, uint16 counts + per-image scale)"}
+                          "h2d_bytes_per_step": int(hr.numel() * 2 + hsc.numel() * 4), "d2h_bytes_per_step": d2h,
+                          "api": "apic_submit_host_u16 / apic_wait_host (uint16 counts + per-image scale, two batches in flight)"}
+            dt = timed(lambda i: plan.reconstruct_host_u16(hr, hsc, hf, hz, hp, hs, stream))
+            e2e["u16"]["single_call"] = {"value": world * k2 * tiles * on * on / 1e6 / dt, "unit": UNIT,
+                                         "api": "apic_reconstruct_host_u16 (blocking)"}
 
     # ---- the oracle on this box's host cores (rank 0, N = 1 only): one tile of the same workload
     cpu = None

@@ -182,6 +182,23 @@ int apic_reconstruct_host_u16(apic_plan* plan, const uint16_t* h_raw, const floa
                               float* h_field, float* h_zernike, float* h_pupil, int32_t* h_status,
                               void* cuda_stream);
 
+/* Streaming form of the host entries, for a sequence of batches (a slide is thousands of tiles,
+ * PAPER.md:177-179): apic_submit_host[_u16] enqueues the upload, the kernels and the download of one
+ * batch in pipeline slot `slot` (0 or 1) and returns without waiting; apic_wait_host(plan, slot)
+ * blocks until that batch's results are in its host buffers and returns its status.  With one
+ * batch in flight per slot the upload of batch k+1 and the download of batch k-1 overlap the
+ * kernels of batch k, so a long sequence runs at max(upload, kernels, download) per batch instead of
+ * their sum.  The host buffers should be pinned (pageable memory makes the copies synchronous) and
+ * must stay valid and untouched until the wait returns; a slot must be waited for before it is
+ * submitted to again (a busy slot is waited for implicitly).  Results are the bits of
+ * apic_reconstruct on the same inputs.  With bg_mode != 0 a submit blocks until the batch's
+ * background pass has run (see apic_reconstruct).  Not thread-safe per plan. */
+int apic_submit_host(apic_plan* plan, int slot, const float* h_intensity, int batch, float* h_field,
+                     float* h_zernike, float* h_pupil, int32_t* h_status);
+int apic_submit_host_u16(apic_plan* plan, int slot, const uint16_t* h_raw, const float* h_scale, int batch,
+                         float* h_field, float* h_zernike, float* h_pupil, int32_t* h_status);
+int apic_wait_host(apic_plan* plan, int slot);
+
 /* Stage-level access for parity tests (device pointers, valid after apic_reconstruct on the
  * same stream, for the tiles of the LAST internal chunk; tile index is chunk-local):
  *   APIC_DBG_SUBSPECTRA: [chunk][sum_i |D_i|] complex64, S_hat_i on D_i (Eq. 7), LED-major, bins

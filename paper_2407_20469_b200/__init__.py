@@ -22,6 +22,7 @@ DBG_SUBSPECTRA, DBG_OBJECT_SPECTRUM, DBG_DF_ITERS = 0, 1, 2
 
 EXPORTS = ("apic_params_default", "apic_plan_create", "apic_plan_destroy", "apic_plan_info",
            "apic_geometry_info", "apic_geometry_dark_grids", "apic_plan_dark_sets", "apic_reconstruct", "apic_reconstruct_host", "apic_reconstruct_u16", "apic_reconstruct_host_u16",
+           "apic_submit_host", "apic_submit_host_u16", "apic_wait_host",
            "apic_debug_buffer", "apic_debug_copy", "apic_fft2d", "apic_fft2d_xy", "apic_last_launch_count", "apic_strerror",
            "apic_last_cuda_error", "apic_version", "apic_profile_categories", "apic_profile_category_name",
            "apic_profile_begin", "apic_profile_end", "apic_profile_work", "apic_measure_peak")
@@ -79,6 +80,10 @@ def load() -> C.CDLL:
     lib.apic_reconstruct_u16.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
                                          C.c_void_p, C.c_void_p]
     lib.apic_reconstruct_host_u16.argtypes = lib.apic_reconstruct_u16.argtypes
+    lib.apic_submit_host.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.apic_submit_host_u16.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p,
+                                         C.c_void_p, C.c_void_p]
+    lib.apic_wait_host.argtypes = [C.c_void_p, C.c_int]
     lib.apic_debug_buffer.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)]
     lib.apic_debug_copy.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p]
     lib.apic_fft2d.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
@@ -274,6 +279,23 @@ class Plan:
                             + self._host_outputs(b, field, zern, pupil, status))
         _check(self._lib.apic_reconstruct_host(self._h, p[0], b, p[1], p[2], p[3], p[4], C.c_void_p(stream)),
                "apic_reconstruct_host")
+
+    def submit_host(self, slot: int, intensity, field, zern, pupil, status):
+        """Streaming form of reconstruct_host: enqueues upload, kernels and download of one batch in pipeline slot
+        0 or 1 and returns; wait_host(slot) blocks until the results are in the (pinned) host buffers."""
+        b = int(intensity.shape[0])
+        p = self._host_ptrs(b, [("intensity", intensity, np.float32, (b, self.n_img, self.n, self.n))]
+                            + self._host_outputs(b, field, zern, pupil, status))
+        _check(self._lib.apic_submit_host(self._h, slot, p[0], b, p[1], p[2], p[3], p[4]), "apic_submit_host")
+
+    def submit_host_u16(self, slot: int, raw, scale, field, zern, pupil, status):
+        b = int(raw.shape[0])
+        p = self._host_ptrs(b, [("raw", raw, np.uint16, (b, self.n_img, self.n, self.n)),
+                                ("scale", scale, np.float32, (b, self.n_img))] + self._host_outputs(b, field, zern, pupil, status))
+        _check(self._lib.apic_submit_host_u16(self._h, slot, p[0], p[1], b, p[2], p[3], p[4], p[5]), "apic_submit_host_u16")
+
+    def wait_host(self, slot: int):
+        _check(self._lib.apic_wait_host(self._h, slot), "apic_wait_host")
 
     def debug_buffer(self, which: int, tiles: int):
         """Stage-level buffers of the last chunk as torch tensors (copies)."""

@@ -59,6 +59,19 @@ struct apic_plan {
   uint16_t* st_raw = nullptr;        // staging of apic_reconstruct_host_u16
   float* st_scale = nullptr;
   int st_raw_batch = 0, st_int_batch = 0;
+  // apic_submit_host / apic_wait_host: one pipeline slot per workspace set
+  struct HostSlot {
+    float* in_f32 = nullptr;
+    uint16_t* in_u16 = nullptr;
+    float* in_scale = nullptr;
+    float *field = nullptr, *zern = nullptr, *pupil = nullptr;
+    int32_t* status = nullptr;
+    int cap_f32 = 0, cap_u16 = 0, cap_out = 0;
+    bool has_pupil = false, busy = false;
+    int rc = 0;
+    cudaStream_t ks = nullptr;
+    cudaEvent_t in_done = nullptr, k_done = nullptr, out_done = nullptr;
+  } slot[2];
   // apic_reconstruct_host: copy streams, a second compute stream and per-part events (upload done, kernels done)
   static constexpr int kMaxParts = 8;
   cudaStream_t copy_in = nullptr, copy_out = nullptr, aux = nullptr;
@@ -222,6 +235,12 @@ int apic_plan_destroy(apic_plan* plan) {
   cudaFree(plan->st_int); cudaFree(plan->st_field); cudaFree(plan->st_zern); cudaFree(plan->st_pupil);
   cudaFree(plan->st_status);
   cudaFree(plan->st_raw); cudaFree(plan->st_scale);
+  for (auto& q : plan->slot) {
+    if (q.busy) cudaEventSynchronize(q.out_done);
+    cudaFree(q.in_f32); cudaFree(q.in_u16); cudaFree(q.in_scale); cudaFree(q.field); cudaFree(q.zern); cudaFree(q.pupil);
+    cudaFree(q.status);
+    if (q.ks) { cudaStreamDestroy(q.ks); cudaEventDestroy(q.in_done); cudaEventDestroy(q.k_done); cudaEventDestroy(q.out_done); }
+  }
   if (plan->copy_in) {
     cudaStreamDestroy(plan->copy_in); cudaStreamDestroy(plan->copy_out); cudaStreamDestroy(plan->aux);
     for (cudaEvent_t e : plan->part_ev) if (e) cudaEventDestroy(e);
@@ -459,6 +478,7 @@ int apic_reconstruct_host_u16(apic_plan* plan, const uint16_t* h_raw, const floa
   return reconstruct_host_impl(plan, nullptr, h_raw, h_scale, batch, h_field, h_zernike, h_pupil, h_status, cuda_stream);
 }
 
+static bool ensure_copy_streams(apic_plan* plan);
 static int reconstruct_host_impl(apic_plan* plan, const float* h_intensity, const uint16_t* h_raw, const float* h_scale,
                                  int batch, float* h_field, float* h_zernike, float* h_pupil, int32_t* h_status,
                                  void* cuda_stream) {
@@ -500,14 +520,9 @@ static int reconstruct_host_impl(apic_plan* plan, const float* h_intensity, cons
     plan->st_int_batch = batch;
   }
   constexpr int kEv = 2 * apic_plan::kMaxParts;
-  if (!plan->copy_in) {
-    bool ok = cuda_ok(cudaStreamCreateWithFlags(&plan->copy_in, cudaStreamNonBlocking), "cudaStreamCreate") &&
-              cuda_ok(cudaStreamCreateWithFlags(&plan->copy_out, cudaStreamNonBlocking), "cudaStreamCreate") &&
-              cuda_ok(cudaStreamCreateWithFlags(&plan->aux, cudaStreamNonBlocking), "cudaStreamCreate");
-    for (int k = 0; ok && k < kEv + 2; ++k)
-      ok = cuda_ok(cudaEventCreateWithFlags(&plan->part_ev[k], cudaEventDisableTiming), "cudaEventCreate");
-    if (!ok) return APIC_ECUDA;
-  }
+  if (!ensure_copy_streams(plan)) return APIC_ECUDA;
+  for (int q = 0; q < 2; ++q)                             // the synchronous entry shares the workspace sets with the slots
+    if (plan->slot[q].busy && apic_wait_host(plan, q) != APIC_OK) return APIC_ECUDA;
   // Sub-batches of >= 16 tiles alternate between the plan's two workspace sets and two compute streams (the caller's
   // and one of the plan's), so that the kernels of part k run beside those of part k+1 and beside the upload of the
   // parts after it and the download of the parts before it.  Results do not depend on the split (a tile's result is
@@ -563,6 +578,112 @@ static int reconstruct_host_impl(apic_plan* plan, const float* h_intensity, cons
   ok = cuda_ok(cudaStreamSynchronize(s), "apic_reconstruct_host") && ok;
   if (rc != APIC_OK) return rc;
   return ok ? APIC_OK : APIC_ECUDA;
+}
+
+// ------------------------------------------------------------------ streaming host entries
+static bool ensure_copy_streams(apic_plan* plan) {
+  constexpr int kEv = 2 * apic_plan::kMaxParts;
+  if (plan->copy_in) return true;
+  bool ok = cuda_ok(cudaStreamCreateWithFlags(&plan->copy_in, cudaStreamNonBlocking), "cudaStreamCreate") &&
+            cuda_ok(cudaStreamCreateWithFlags(&plan->copy_out, cudaStreamNonBlocking), "cudaStreamCreate") &&
+            cuda_ok(cudaStreamCreateWithFlags(&plan->aux, cudaStreamNonBlocking), "cudaStreamCreate");
+  for (int k = 0; ok && k < kEv + 2; ++k)
+    ok = cuda_ok(cudaEventCreateWithFlags(&plan->part_ev[k], cudaEventDisableTiming), "cudaEventCreate");
+  return ok;
+}
+
+static bool grow_bytes(void** p, size_t bytes) {
+  cudaFree(*p);
+  *p = nullptr;
+  return cuda_ok(cudaMalloc(p, bytes), "cudaMalloc staging");
+}
+#define grow(pp, count) grow_bytes(reinterpret_cast<void**>(pp), (count) * sizeof(**(pp)))
+
+static int submit_host_impl(apic_plan* plan, int slot, const float* h_intensity, const uint16_t* h_raw, const float* h_scale,
+                            int batch, float* h_field, float* h_zernike, float* h_pupil, int32_t* h_status) {
+  if (!plan || !h_field || !h_zernike || !h_status || slot < 0 || slot > 1) return APIC_EINVAL;
+  if (batch < 1 || batch > plan->params.max_batch) return APIC_EBATCH;
+  DeviceGuard guard(plan->pd.device);
+  apic_plan::HostSlot& q = plan->slot[slot];
+  if (q.busy) {                                          // a slot holds one batch at a time
+    const int rc = apic_wait_host(plan, slot);
+    if (rc != APIC_OK) return rc;
+  }
+  const DevTables& t = plan->dev;
+  const size_t nn = size_t(t.n) * t.n, on = size_t(t.n) * t.u, img_px = size_t(t.n_img) * nn;
+  if (!ensure_copy_streams(plan)) return APIC_ECUDA;
+  if (!plan->alloc_set(plan->set[slot])) return APIC_ENOMEM;
+  if (!q.ks) {
+    bool ok = cuda_ok(cudaStreamCreateWithFlags(&q.ks, cudaStreamNonBlocking), "cudaStreamCreate") &&
+              cuda_ok(cudaEventCreateWithFlags(&q.in_done, cudaEventDisableTiming), "cudaEventCreate") &&
+              cuda_ok(cudaEventCreateWithFlags(&q.k_done, cudaEventDisableTiming), "cudaEventCreate") &&
+              cuda_ok(cudaEventCreateWithFlags(&q.out_done, cudaEventDisableTiming), "cudaEventCreate");
+    if (!ok) return APIC_ECUDA;
+    cudaEventRecord(q.k_done, q.ks);                     // "the previous batch of this slot has read its inputs"
+  }
+  // staging buffers of this slot (grow-only; the slot is idle here, so nothing reads the old ones)
+  if (batch > q.cap_out || (h_pupil && !q.has_pupil)) {
+    bool ok = grow(&q.field, size_t(batch) * on * on * 2) && grow(&q.zern, size_t(batch) * t.nz) &&
+              grow(&q.status, size_t(batch));
+    if (ok && (h_pupil || q.has_pupil)) ok = grow(&q.pupil, size_t(batch) * nn * 2);
+    if (!ok) { q.cap_out = 0; return APIC_ENOMEM; }
+    q.cap_out = batch;
+    q.has_pupil = q.has_pupil || h_pupil != nullptr;
+  }
+  if (h_raw && batch > q.cap_u16) {
+    if (!grow(&q.in_u16, size_t(batch) * img_px) || !grow(&q.in_scale, size_t(batch) * t.n_img)) { q.cap_u16 = 0; return APIC_ENOMEM; }
+    q.cap_u16 = batch;
+  }
+  if (!h_raw && batch > q.cap_f32) {
+    if (!grow(&q.in_f32, size_t(batch) * img_px)) { q.cap_f32 = 0; return APIC_ENOMEM; }
+    q.cap_f32 = batch;
+  }
+  // upload (one copy stream for both slots: uploads queue behind each other and beside the other slot's kernels)
+  cudaStreamWaitEvent(plan->copy_in, q.k_done, 0);
+  if (h_raw) {
+    cudaMemcpyAsync(q.in_u16, h_raw, size_t(batch) * img_px * sizeof(uint16_t), cudaMemcpyHostToDevice, plan->copy_in);
+    cudaMemcpyAsync(q.in_scale, h_scale, size_t(batch) * t.n_img * sizeof(float), cudaMemcpyHostToDevice, plan->copy_in);
+  } else {
+    cudaMemcpyAsync(q.in_f32, h_intensity, size_t(batch) * img_px * sizeof(float), cudaMemcpyHostToDevice, plan->copy_in);
+  }
+  cudaEventRecord(q.in_done, plan->copy_in);
+  // kernels
+  cudaStreamWaitEvent(q.ks, q.in_done, 0);
+  const ImgSrc src = h_raw ? ImgSrc{nullptr, q.in_u16, q.in_scale} : ImgSrc{q.in_f32, nullptr, nullptr};
+  float* pu = h_pupil ? q.pupil : nullptr;
+  const int rc = reconstruct_impl(plan, slot, src, batch, q.field, q.zern, pu, q.status, q.ks);
+  cudaEventRecord(q.k_done, q.ks);
+  if (rc != APIC_OK) { cudaStreamSynchronize(q.ks); return rc; }
+  // download
+  cudaStreamWaitEvent(plan->copy_out, q.k_done, 0);
+  cudaMemcpyAsync(h_field, q.field, size_t(batch) * on * on * 2 * sizeof(float), cudaMemcpyDeviceToHost, plan->copy_out);
+  cudaMemcpyAsync(h_zernike, q.zern, size_t(batch) * t.nz * sizeof(float), cudaMemcpyDeviceToHost, plan->copy_out);
+  if (h_pupil) cudaMemcpyAsync(h_pupil, pu, size_t(batch) * nn * 2 * sizeof(float), cudaMemcpyDeviceToHost, plan->copy_out);
+  cudaMemcpyAsync(h_status, q.status, size_t(batch) * sizeof(int32_t), cudaMemcpyDeviceToHost, plan->copy_out);
+  cudaEventRecord(q.out_done, plan->copy_out);
+  q.busy = true;
+  return cuda_ok(cudaGetLastError(), "apic_submit_host") ? APIC_OK : APIC_ECUDA;
+}
+
+int apic_submit_host(apic_plan* plan, int slot, const float* h_intensity, int batch, float* h_field, float* h_zernike,
+                     float* h_pupil, int32_t* h_status) {
+  if (!h_intensity) return APIC_EINVAL;
+  return submit_host_impl(plan, slot, h_intensity, nullptr, nullptr, batch, h_field, h_zernike, h_pupil, h_status);
+}
+
+int apic_submit_host_u16(apic_plan* plan, int slot, const uint16_t* h_raw, const float* h_scale, int batch, float* h_field,
+                         float* h_zernike, float* h_pupil, int32_t* h_status) {
+  if (!h_raw || !h_scale) return APIC_EINVAL;
+  return submit_host_impl(plan, slot, nullptr, h_raw, h_scale, batch, h_field, h_zernike, h_pupil, h_status);
+}
+
+int apic_wait_host(apic_plan* plan, int slot) {
+  if (!plan || slot < 0 || slot > 1) return APIC_EINVAL;
+  apic_plan::HostSlot& q = plan->slot[slot];
+  if (!q.busy) return APIC_OK;
+  DeviceGuard guard(plan->pd.device);
+  q.busy = false;
+  return cuda_ok(cudaEventSynchronize(q.out_done), "apic_wait_host") ? APIC_OK : APIC_ECUDA;
 }
 
 int apic_debug_buffer(const apic_plan* plan, int which, void** d_ptr, size_t* bytes_per_tile) {

@@ -539,6 +539,53 @@ def test_host_entry_pipelines_sub_batches_without_changing_bits(A):
     assert np.array_equal(field[0], field[4]) and np.array_equal(field[1], field[69])
 
 
+def test_streaming_host_entry_keeps_two_batches_in_flight_without_changing_bits(A):
+    """apic_submit_host / apic_wait_host: a sequence of different batches through the two pipeline slots (pinned
+    buffers; fp32 and uint16 inputs; a slot reused without an explicit wait; ragged batch sizes) gives the bits of
+    the device entry on each batch."""
+    import torch
+    cfg = get_config(2, tile_n=64, batch=4, grid=(2, 2))
+    stacks, truths = make_batch(cfg, [0, 1, 2, 3])
+    plan = plan_from_config(A, cfg, max_batch=12)
+    batches = [np.ascontiguousarray(np.concatenate([stacks[i:], stacks[:i]] * 3)[:nb]) for i, nb in ((0, 12), (1, 7), (2, 12), (3, 5))]
+    refs = [[o.cpu().numpy() for o in plan.reconstruct(torch.from_numpy(b).cuda())] for b in batches]
+    torch.cuda.synchronize()
+    nz, n, on = plan.nz, plan.n, plan.out_n
+    bufs = []
+    for b in batches:
+        nb = len(b)
+        bufs.append((torch.from_numpy(b).pin_memory(), torch.zeros((nb, on, on), dtype=torch.complex64).pin_memory(),
+                     torch.zeros((nb, nz), dtype=torch.float32).pin_memory(),
+                     torch.zeros((nb, n, n), dtype=torch.complex64).pin_memory(),
+                     torch.full((nb,), -1, dtype=torch.int32).pin_memory()))
+    for k, (x, f, z, p, s) in enumerate(bufs):                     # slots 0, 1, 0, 1: the third submit finds slot 0 busy
+        plan.submit_host(k & 1, x, f, z, p, s)
+    plan.wait_host(0)
+    plan.wait_host(1)
+    for (x, f, z, p, s), ref in zip(bufs, refs):
+        assert np.array_equal(f.numpy(), ref[0]) and np.array_equal(z.numpy(), ref[1])
+        assert np.array_equal(p.numpy(), ref[2]) and np.array_equal(s.numpy(), ref[3])
+    # uint16 counts + per-image scale through the same slots, interleaved with the blocking entry
+    gains = np.array([[t.gain_bright] * cfg.n_bright + [t.gain_dark] * cfg.n_dark for t in truths])
+    raw = np.rint(stacks.astype(np.float64) * gains[:, :, None, None]).astype(np.uint16)
+    scale = (1.0 / gains).astype(np.float32)
+    ref16 = [o.cpu().numpy() for o in plan.reconstruct_u16(torch.from_numpy(raw).cuda(), torch.from_numpy(scale).cuda())]
+    torch.cuda.synchronize()
+    hr, hsc = torch.from_numpy(raw).pin_memory(), torch.from_numpy(scale).pin_memory()
+    o16 = [(torch.zeros((4, on, on), dtype=torch.complex64).pin_memory(), torch.zeros((4, nz), dtype=torch.float32).pin_memory(),
+            torch.zeros((4, n, n), dtype=torch.complex64).pin_memory(), torch.zeros((4,), dtype=torch.int32).pin_memory())
+           for _ in range(2)]
+    plan.submit_host_u16(1, hr, hsc, *o16[1])
+    plan.submit_host_u16(0, hr, hsc, *o16[0])
+    f2 = np.zeros_like(refs[1][0]); z2 = np.zeros_like(refs[1][1]); p2 = np.zeros_like(refs[1][2]); s2 = np.zeros_like(refs[1][3])
+    plan.reconstruct_host(batches[1], f2, z2, p2, s2)              # waits for both slots, then runs
+    assert np.array_equal(f2, refs[1][0]) and np.array_equal(s2, refs[1][3])
+    plan.wait_host(0)
+    plan.wait_host(1)
+    for o in o16:
+        assert np.array_equal(o[0].numpy(), ref16[0]) and np.array_equal(o[1].numpy(), ref16[1])
+
+
 def test_config4_full_tile_size_with_background_tiles(A):
     """Config 4's tiles at full size (256 x 256, 8 + 16 LEDs, the reduced-grid darkfield kernel) with
     blank tiles in the batch: statuses of every tile, zero outputs for the skipped ones, one live tile
