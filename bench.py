@@ -58,6 +58,12 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--breakdown", action="store_true", help="also print the per-kernel time table to stderr")
+    ap.add_argument("--ncu-summary", default="", help="no run: append the kernels of an `ncu -i <rep> --page raw --csv` dump "
+                    "to profiles/r2_ncu_kernels.csv (with --commit and --workload)")
+    ap.add_argument("--commit", default="", help="--ncu-summary: the commit the capture was taken at")
+    ap.add_argument("--workload", default="", help="--ncu-summary: workload tag, e.g. cfg2_64tiles")
+    ap.add_argument("--dense-probe", action="store_true", help="no run of the library: time the dense route of the darkfield "
+                    "step (G = C^H C with the library GEMM on tensor cores) for the shapes of config 2")
     return ap.parse_args()
 
 
@@ -169,7 +175,7 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------ roofline helpers
-KERNEL_SOURCES = ("df_mgrid.cu", "df_team.cu", "fft_xy.cuh", "fft_core.cuh")
+KERNEL_SOURCES = ("df_mgrid.cu", "df_tma.cu", "df_team.cu", "fft_xy.cuh", "fft_core.cuh")
 
 
 def kernel_source_hash():
@@ -200,6 +206,112 @@ def ncu_capture(kernel, workload):
             "smem_wavefronts": int(r["smem_wavefronts"]), "duration_ms": float(r["duration_ms"]), "commit": r["commit"]}
 
 
+def ncu_summary(args):
+    """Reduces an `ncu --page raw --csv` dump of an `ncu --set full` capture to one row per kernel launch in
+    profiles/r2_ncu_kernels.csv: what bench.py's roofline line reads (traffic, smem_frac) plus the figures DESIGN.md
+    quotes (issue-slot utilisation, occupancy, L2 hit rate, stall shares)."""
+    import csv
+    with open(args.ncu_summary) as fh:
+        rows = list(csv.reader(fh))
+    hdr, units = rows[0], rows[1]
+    ix = {h: i for i, h in enumerate(hdr)}
+
+    def val(r, key, scale_units=True):
+        v = r[ix[key]].replace(",", "")
+        if v in ("", "n/a"):
+            return 0.0
+        x = float(v)
+        u = units[ix[key]]
+        if scale_units:
+            x *= {"Mbyte": 1e6, "Gbyte": 1e9, "Kbyte": 1e3, "byte": 1.0, "us": 1e-3, "ns": 1e-6, "ms": 1.0, "s": 1e3}.get(u, 1.0)
+        return x
+
+    out_path = os.path.join(ROOT, "profiles", "r2_ncu_kernels.csv")
+    fields = ["kernel", "workload", "commit", "source_hash", "duration_ms", "dram_bytes_read", "dram_bytes_write",
+              "smem_wavefronts", "inst_executed", "issue_active_pct", "warps_active_pct", "l2_hit_pct", "registers",
+              "dyn_smem_bytes", "grid", "cluster", "stall_barrier_pct", "stall_long_sb_pct", "stall_short_sb_pct",
+              "stall_wait_pct", "stall_membar_pct"]
+    new = not os.path.exists(out_path)
+    with open(out_path, "a", newline="") as fh:
+        w = csv.DictWriter(fh, fieldnames=fields)
+        if new:
+            w.writeheader()
+        for r in rows[2:]:
+            name = r[ix["Kernel Name"]].split("(")[0].split("::")[-1]
+            stall = {k: val(r, f"smsp__average_warps_issue_stalled_{k}_per_issue_active.ratio", False)
+                     for k in ("barrier", "long_scoreboard", "short_scoreboard", "wait", "membar", "no_instruction", "not_selected",
+                               "selected", "math_pipe_throttle", "mio_throttle", "lg_throttle", "branch_resolving", "dispatch_stall",
+                               "drain", "imc_miss", "sleeping", "tex_throttle", "misc")
+                     if f"smsp__average_warps_issue_stalled_{k}_per_issue_active.ratio" in ix}
+            tot = sum(stall.values()) or 1.0
+            w.writerow({"kernel": name, "workload": args.workload, "commit": args.commit, "source_hash": kernel_source_hash(),
+                        "duration_ms": f"{val(r, 'gpu__time_duration.sum'):.4f}",
+                        "dram_bytes_read": int(val(r, "dram__bytes_read.sum")), "dram_bytes_write": int(val(r, "dram__bytes_write.sum")),
+                        "smem_wavefronts": int(val(r, "l1tex__data_pipe_lsu_wavefronts_mem_shared.sum")),
+                        "inst_executed": int(val(r, "smsp__inst_executed.sum")),
+                        "issue_active_pct": f"{val(r, 'smsp__issue_active.avg.pct_of_peak_sustained_active'):.2f}",
+                        "warps_active_pct": f"{val(r, 'sm__warps_active.avg.pct_of_peak_sustained_active'):.2f}",
+                        "l2_hit_pct": f"{val(r, 'lts__t_sector_hit_rate.pct'):.2f}",
+                        "registers": int(val(r, "launch__registers_per_thread")),
+                        "dyn_smem_bytes": int(val(r, "launch__shared_mem_per_block_dynamic")),
+                        "grid": int(val(r, "launch__grid_size")), "cluster": int(val(r, "launch__cluster_dim_x")),
+                        "stall_barrier_pct": f"{100 * stall.get('barrier', 0) / tot:.1f}",
+                        "stall_long_sb_pct": f"{100 * stall.get('long_scoreboard', 0) / tot:.1f}",
+                        "stall_short_sb_pct": f"{100 * stall.get('short_scoreboard', 0) / tot:.1f}",
+                        "stall_wait_pct": f"{100 * stall.get('wait', 0) / tot:.1f}",
+                        "stall_membar_pct": f"{100 * stall.get('membar', 0) / tot:.1f}"})
+            print("appended", name, args.workload, "to", out_path)
+
+
+def dense_probe():
+    """The dense route of the darkfield step, for DESIGN.md section 7 (north_star: tensor cores only if the contraction
+    dominates): PAPER.md:135 builds the block-Toeplitz C explicitly (|Q| x |U| complex per LED); its normal matrix
+    G = C^H C is a contraction over |Q|.  Times G for ONE darkfield LED of each of 64 tiles with the library GEMM
+    (cuBLAS through torch.bmm; complex = 4 real products) in fp32 and on the tensor cores in TF32 (one pass: 10-bit
+    mantissas, too coarse for the 1e-3 band tolerance; fp32-level accuracy needs 3 passes), plus the Cholesky factor."""
+    import torch
+    torch.cuda.set_device(0)
+
+    def timeit(f, n=5):
+        for _ in range(2):
+            f()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            f()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n
+
+    tiles, res = 64, {}
+    for name, (nq, nu) in {"ring_0.30": (8624, 569), "ring_0.40": (7908, 1194)}.items():   # |Q| x |U| of config 2's plan
+        cr = torch.randn(tiles, nq, nu, device="cuda")
+        ci = torch.randn(tiles, nq, nu, device="cuda")
+        flop = 4 * 2.0 * tiles * nq * nu * nu
+        row = {"Q": nq, "U": nu, "tiles": tiles}
+        for mode, tf32 in (("fp32", False), ("tf32_1pass", True)):
+            torch.backends.cuda.matmul.allow_tf32 = tf32
+
+            def gram():
+                a = torch.bmm(cr.transpose(1, 2), cr)
+                a += torch.bmm(ci.transpose(1, 2), ci)
+                b = torch.bmm(cr.transpose(1, 2), ci)
+                b -= torch.bmm(ci.transpose(1, 2), cr)
+                return a, b
+            ms = timeit(gram)
+            row[mode] = {"ms_per_led": ms, "tflops_real": flop / ms / 1e9}
+        torch.backends.cuda.matmul.allow_tf32 = False
+        g = torch.randn(tiles, nu, nu, dtype=torch.complex64, device="cuda")
+        g = g @ g.conj().transpose(1, 2) + nu * torch.eye(nu, device="cuda", dtype=torch.complex64)
+        row["cholesky_ms_per_led"] = timeit(lambda: torch.linalg.cholesky(g), n=2)
+        res[name] = row
+        del cr, ci, g
+    step = sum(8 * (r["tf32_1pass"]["ms_per_led"] + r["cholesky_ms_per_led"]) for r in res.values())
+    print(json.dumps({"dense_probe": res, "ms_per_64_tile_step_tf32_1pass": step,
+                      "note": "8 LEDs per ring; building C and the right-hand sides not included"}), flush=True)
+
+
 def measured_peaks(A, torch, sm_mhz_max, sms):
     """fp32 FFMA / FADD rates and shared-memory read bandwidth measured on this device now; the derived figures
     (unit counts x clock) beside them."""
@@ -216,6 +328,12 @@ def measured_peaks(A, torch, sm_mhz_max, sms):
 # ------------------------------------------------------------------------------------ product arm
 def main():
     args = parse_args()
+    if args.ncu_summary:
+        ncu_summary(args)
+        return
+    if args.dense_probe:
+        dense_probe()
+        return
     from apic_synth import get_config, make_batch, plan_args
     cfg = get_config(args.config)
     if args.impl == "reference":

@@ -61,6 +61,7 @@ class OracleParams:
     intensity_floor: float = 1e-6
     bg_mode: int = 0
     bg_threshold: float = 0.0
+    dark_order: str = "sequential"         # R15 "sequential" (the contract) | "ring" (second reading R15b)
 
     @property
     def radius(self) -> float:
@@ -207,6 +208,13 @@ class Geometry:
         key = [(int(round(float(np.hypot(*k)) / KAPPA_ORDER_QUANTUM)), i) for i, k in enumerate(self.kappa_d)]
         return [i for _, i in sorted(key)]
 
+    def _dark_rings(self) -> List[List[int]]:
+        """Darkfield LEDs grouped by |kappa| (same rounding as the order), rings in ascending |kappa|."""
+        rings: Dict[int, List[int]] = {}
+        for i in self._dark_order():
+            rings.setdefault(int(round(float(np.hypot(*self.kappa_d[i])) / KAPPA_ORDER_QUANTUM)), []).append(i)
+        return [rings[k] for k in sorted(rings)]
+
     def to_centred(self, a_fft_order: np.ndarray) -> np.ndarray:
         return np.fft.fftshift(a_fft_order, axes=(-2, -1))
 
@@ -241,33 +249,51 @@ class DarkSets:
     U: np.ndarray            # centred bool: D_i \ known
     Q: np.ndarray            # centred bool: linear region
     unknown_fraction: float
+    ring: int = 0            # index of the LED's ring (equal |kappa|), ascending
 
 
 def darkfield_sets(geo: Geometry) -> Tuple[List[DarkSets], np.ndarray]:
     """O6 index sets for every darkfield LED in processing order (Eq. 13 region Q_i,
-    PAPER.md:130-132; R15, R16).  Returns (list, final known mask)."""
+    PAPER.md:130-132; R15, R16).  Returns (list, final known mask).
+
+    PAPER.md:135 extends the spectrum "across all darkfield measurements" without stating an order.
+    R15 (``dark_order = "sequential"``, the contract): one LED after the other, ``known`` grows after
+    every LED, a bin belongs to the first LED that solves it.  R15b (``"ring"``): every LED of a ring
+    (equal |kappa|) is solved against ``known`` as it stands when the ring starts; ``known`` grows once
+    per ring (bins solved by several LEDs of the ring are averaged in darkfield_extend)."""
     known = np.zeros((geo.n, geo.n), dtype=bool)
     for m in geo.disc_b:
         known |= m
+    ring_wise = geo.p.dark_order == "ring"
+    if geo.p.dark_order not in ("sequential", "ring"):
+        raise ValueError("dark_order must be 'sequential' or 'ring'")
     out: List[DarkSets] = []
-    for led in geo.dark_order:
-        d = geo.disc_d[led]
-        P = d & known
-        U = d & ~known
-        if not U.any():
-            continue
-        frac = U.sum() / float(d.sum())
-        if frac > MAX_UNKNOWN_FRACTION:
-            raise ValueError(f"darkfield LED {led}: unknown fraction {frac:.3f} > 0.42 (PAPER.md:201)")
-        cross = minkowski_difference(U, P)          # supp(U ⋆ P) = {u - p}
-        other = minkowski_difference(P, U)          # supp(P ⋆ U) = {p - u}
-        auto = minkowski_difference(U, U)           # supp(U ⋆ U) = {u - u'}
-        Q = cross & ~(other | auto)
-        if not Q.any():
-            raise ValueError(f"darkfield LED {led}: empty linear region Q")
-        out.append(DarkSets(led=led, P=P, U=U, Q=Q, unknown_fraction=frac))
-        known = known | U
+    for ri, ring in enumerate(geo._dark_rings()):
+        start = known.copy()
+        for led in ring:
+            base = start if ring_wise else known
+            d = geo.disc_d[led]
+            P = d & base
+            U = d & ~base
+            if not U.any():
+                continue
+            known = _dark_sets_one(out, led, ri, d, P, U, known)
     return out, known
+
+
+def _dark_sets_one(out, led, ring, d, P, U, known):
+    """Checks and the linear region Q of one LED (Eq. 13; R16); appends to ``out`` and returns known ∪ U."""
+    frac = U.sum() / float(d.sum())
+    if frac > MAX_UNKNOWN_FRACTION:
+        raise ValueError(f"darkfield LED {led}: unknown fraction {frac:.3f} > 0.42 (PAPER.md:201)")
+    cross = minkowski_difference(U, P)          # supp(U ⋆ P) = {u - p}
+    other = minkowski_difference(P, U)          # supp(P ⋆ U) = {p - u}
+    auto = minkowski_difference(U, U)           # supp(U ⋆ U) = {u - u'}
+    Q = cross & ~(other | auto)
+    if not Q.any():
+        raise ValueError(f"darkfield LED {led}: empty linear region Q")
+    out.append(DarkSets(led=led, P=P, U=U, Q=Q, unknown_fraction=frac, ring=ring))
+    return known | U
 
 
 # ----------------------------------------------------------------------------------------------
@@ -492,22 +518,39 @@ def darkfield_extend(geo: Geometry, o_hat: np.ndarray, known: np.ndarray, coef: 
         sets, _ = darkfield_sets(geo)
     o_hat = o_hat.copy()
     known = known.copy()
-    for ds in sets:
-        kap = geo.kappa_d[ds.led]
-        if not np.array_equal(ds.P, geo.disc_d[ds.led] & known):
-            raise AssertionError("darkfield index sets out of sync with the known region")
-        phi = pupil_phase(p.noll, coef, geo.kx, geo.ky, kap, geo.radius)
-        p_hat = np.where(ds.P, o_hat * np.exp(1j * phi), 0.0)
-        spec_i = np.fft.fftshift(fft2n(np.asarray(dark_stack[ds.led], dtype=np.float64)))
-        rhs_grid = spec_i - correlate_fft(p_hat, p_hat)                   # Eq. 13 lhs
-        d = rhs_grid[ds.Q]
-        cmat = darkfield_matrix(p_hat, ds.P, ds.U, ds.Q)
-        u_hat, *_ = np.linalg.lstsq(cmat, d, rcond=None)
-        o_hat[ds.U] = u_hat * np.exp(-1j * phi[ds.U])
-        known = known | ds.U
-        if collect is not None:
-            collect.append(dict(led=ds.led, u_hat=u_hat, d=d, p_hat=p_hat,
-                                resid=float(np.linalg.norm(cmat @ u_hat - d) / max(np.linalg.norm(d), 1e-300))))
+    ring_wise = p.dark_order == "ring"
+    for ri in sorted({ds.ring for ds in sets}):
+        ring = [ds for ds in sets if ds.ring == ri]
+        # R15b: every LED of the ring reads the spectrum and the known set as they stand when the ring starts;
+        # a bin solved by several LEDs of the ring gets the unweighted mean of their solutions (the rule of R13)
+        o_start, known_start = o_hat.copy(), known.copy()
+        acc = np.zeros_like(o_hat)
+        cnt = np.zeros(o_hat.shape, dtype=np.int64)
+        for ds in ring:
+            o_src, k_src = (o_start, known_start) if ring_wise else (o_hat, known)
+            kap = geo.kappa_d[ds.led]
+            if not np.array_equal(ds.P, geo.disc_d[ds.led] & k_src):
+                raise AssertionError("darkfield index sets out of sync with the known region")
+            phi = pupil_phase(p.noll, coef, geo.kx, geo.ky, kap, geo.radius)
+            p_hat = np.where(ds.P, o_src * np.exp(1j * phi), 0.0)
+            spec_i = np.fft.fftshift(fft2n(np.asarray(dark_stack[ds.led], dtype=np.float64)))
+            rhs_grid = spec_i - correlate_fft(p_hat, p_hat)                   # Eq. 13 lhs
+            d = rhs_grid[ds.Q]
+            cmat = darkfield_matrix(p_hat, ds.P, ds.U, ds.Q)
+            u_hat, *_ = np.linalg.lstsq(cmat, d, rcond=None)
+            if ring_wise:
+                acc[ds.U] += u_hat * np.exp(-1j * phi[ds.U])
+                cnt[ds.U] += 1
+            else:
+                o_hat[ds.U] = u_hat * np.exp(-1j * phi[ds.U])
+                known = known | ds.U
+            if collect is not None:
+                collect.append(dict(led=ds.led, u_hat=u_hat, d=d, p_hat=p_hat,
+                                    resid=float(np.linalg.norm(cmat @ u_hat - d) / max(np.linalg.norm(d), 1e-300))))
+        if ring_wise:
+            solved = cnt > 0
+            o_hat[solved] = acc[solved] / cnt[solved]
+            known = known | solved
     return o_hat, known
 
 
