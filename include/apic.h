@@ -71,7 +71,11 @@ typedef struct {
   int n_zernike;         /* number of fitted Zernike terms (1..64)                               */
   const int* noll;       /* host, [n_zernike] distinct Noll indices, each >= 4 (piston and tilts
                             are the exact null space of Eq. 10; R9)                    */
-  int kk_pad;            /* Fourier pre-upsampling of I before the log: only 1 is implemented     */
+  int kk_pad;            /* 1 or 2 (2: tile_n <= 256).  The log of Eq. 5 is not band-limited; with 2
+                            every NA-matching image is Fourier-interpolated to the 2N grid before
+                            the log and the KK chain runs there, which removes the aliasing floor
+                            of the retrieved field (2e-4 -> 4e-9 on config 0; R7) at 4x
+                            the transform work of S1-S5                                          */
   int refine_iters;      /* re-wrapped refinements of the aberration fit (R11); 0..16   */
   int df_iters;          /* maximum CGLS iterations per darkfield LED (>= 1)                      */
   float df_tol;          /* CGLS stops when ||C^H r|| <= df_tol * ||C^H d||; 0 = run df_iters     */
@@ -96,6 +100,13 @@ typedef struct {
                             team (N = 256; other N fall back to the full-grid team kernel)      */
   int df_team;           /* CTAs per tile, 1..8; 0 = chosen from the pass size (as many as the
                             pass leaves resident CTA slots for)                                 */
+  int df_order;          /* order of the darkfield extension (PAPER.md:135 states none).  0 = one
+                            LED after the other by ascending |kappa|, ties by input order; a bin
+                            belongs to the first LED that solves it (reading R15, the default).
+                            1 = ring-wise (reading R15b): every LED of a ring (equal |kappa|) is
+                            solved against the known set as it stands when the ring starts, bins
+                            solved by several LEDs of the ring get the mean of their solutions,
+                            the known set grows once per ring                                   */
 } apic_params;
 
 /* Fills *p with the defaults (kk_pad 1, refine_iters 3, df_iters 48, df_tol 1e-4, floor 1e-6,
@@ -108,7 +119,7 @@ void apic_params_default(apic_params* p);
  * The arrays inside *p are copied.  APIC_EINVAL if: N not in {64,128,256,512}; u outside 1..4;
  * an NA-matching LED with | |kappa_i| - R | > 0.5 bin; the synthetic aperture does not fit the raw
  * grid (max|kappa| + R >= N/2 - 1); a darkfield LED whose unknown fraction exceeds 42 %
- * or whose linear region Q is empty; a Noll index < 4 or repeated; kk_pad != 1; fewer than one
+ * or whose linear region Q is empty; a Noll index < 4 or repeated; kk_pad not 1 or 2; fewer than one
  * overlapping pair. */
 int apic_plan_create(const apic_params* p, apic_plan** out);
 int apic_plan_destroy(apic_plan* plan);

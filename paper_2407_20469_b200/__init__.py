@@ -39,7 +39,8 @@ class ApicParams(C.Structure):
                 ("n_zernike", C.c_int), ("noll", C.POINTER(C.c_int)), ("kk_pad", C.c_int),
                 ("refine_iters", C.c_int), ("df_iters", C.c_int), ("df_tol", C.c_float),
                 ("intensity_floor", C.c_float), ("bg_mode", C.c_int), ("bg_threshold", C.c_float),
-                ("max_batch", C.c_int), ("chunk_tiles", C.c_int), ("df_mode", C.c_int), ("df_team", C.c_int)]
+                ("max_batch", C.c_int), ("chunk_tiles", C.c_int), ("df_mode", C.c_int), ("df_team", C.c_int),
+                ("df_order", C.c_int)]
 
 
 class PlanInfo(C.Structure):
@@ -115,7 +116,7 @@ def _check(rc: int, what: str):
 def make_params(tile_n: int, upsample: int, wavelength_um: float, pixel_um: float, na_obj: float,
                 k_bright, k_dark, noll: Sequence[int], **opts):
     """Returns (ApicParams, keep-alive tuple).  ``opts``: kk_pad, refine_iters, df_iters, df_tol,
-    intensity_floor, bg_mode, bg_threshold, max_batch, chunk_tiles, df_mode, df_team."""
+    intensity_floor, bg_mode, bg_threshold, max_batch, chunk_tiles, df_mode, df_team, df_order."""
     lib = load()
     p = ApicParams()
     lib.apic_params_default(C.byref(p))

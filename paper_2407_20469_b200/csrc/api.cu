@@ -113,7 +113,9 @@ bool apic_plan::alloc_set(WsSet& z) {
   w.gram_parts = (std::max(d.n_rows, d.n_grad) + kGramRows - 1) / kGramRows;
   const size_t n_led = std::max<size_t>(1, h.dark.size());
   bool ok = true;
-  ok = ok && dalloc(&w.G, c * h.nb * nn, false);
+  ok = ok && dalloc(&w.G, c * h.nb * size_t(h.kk_n) * h.kk_n, false);
+  w.KP = nullptr;
+  if (h.kk_n != h.n) ok = ok && dalloc(&w.KP, c * h.nb * nn, false);
   ok = ok && dalloc(&w.S, c * d.disc_total, false);
   ok = ok && dalloc(&w.PR, c * d.n_rows, false);
   ok = ok && dalloc(&w.gram, c * w.gram_parts * w.gram_entries, false);
@@ -183,6 +185,7 @@ void apic_params_default(apic_params* p) {
   p->chunk_tiles = 0;
   p->df_mode = 0;
   p->df_team = 0;
+  p->df_order = 0;
 }
 
 const char* apic_strerror(int err) {
@@ -280,6 +283,13 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
     std::vector<float2> tw;
     build_twiddles(n, tw);
     ok = ok && plan->upload(&d.tw, tw);
+    d.kk_n = h.kk_n;
+    d.tw_kk = d.tw;
+    if (h.kk_n != n) {
+      std::vector<float2> twk;
+      build_twiddles(h.kk_n, twk);
+      ok = ok && plan->upload(&d.tw_kk, twk);
+    }
     std::vector<float2> txy, one;
     for (int r1 : {6, 8, 10, 12, 16}) {
       build_twiddles_xy(r1, one);
@@ -340,6 +350,10 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
     for (int st = 0; st <= kMaxUStrips; ++st)
       q.u_strip_off[st] = L.u_row_off[size_t(std::min(16 * st, L.u_nrow))];
     if ((L.u_nrow + 15) / 16 > kMaxUStrips) ok = false;
+    q.accumulate = L.accumulate ? 1 : 0;
+    q.n_avg = int(L.avg_f.size());
+    ok = ok && plan->upload(&q.avg_f, L.avg_f);
+    ok = ok && plan->upload(&q.avg_w, L.avg_w);
     auto modp = [](int k, int m) { return ((k % m) + m) % m; };
     q.u0m = modp(L.u_row0, L.my); q.q0m = modp(L.q_row0, L.my); q.d0m = modp(L.d_row0, L.my);
     ok = ok && plan->upload(&q.dmap_m, L.dmap_m);

@@ -599,11 +599,21 @@ __global__ void __launch_bounds__(mg::TH, 2) df_mgrid_kernel(const __grid_consta
           const float phi = zern_phase(Lsh.zern + size_t(e) * nz, c_sh, nz);
           float sn, cs;
           sincosf(phi, &sn, &cs);
-          o[Lsh.disc_f[e]] = cmulc(c.xs()[e], make_float2(cs, sn));
+          const int q = Lsh.disc_f[e];
+          const float2 u = cmulc(c.xs()[e], make_float2(cs, sn));
+          o[q] = Lsh.accumulate ? cadd(__ldcg(&o[q]), u) : u;   // ring-wise order (R15b): sum now, mean at the end of the ring
         }
         if (g == 0 && threadIdx.x == 0) a.cg_iters[size_t(slot) * a.n_leds + k] = iters;
       }
       team_sync(multi);                                    // O complete before the next LED reads it
+      if (Lsh.n_avg > 0) {                                 // df_order 1, end of a ring: bins solved by c LEDs hold a sum of c solutions
+        float2* o = a.O + size_t(slot) * (N * N);
+        for (int i = int(g) * TH + threadIdx.x; i < Lsh.n_avg; i += int(G) * TH) {
+          const int q = __ldg(&Lsh.avg_f[i]);
+          o[q] = cscale(__ldcg(&o[q]), __ldg(&Lsh.avg_w[i]));
+        }
+        team_sync(multi);
+      }
     }
   }
   if (threadIdx.x == 0 && flop > 0.0) atomicAdd(a.work, (unsigned long long)(flop + 0.5));

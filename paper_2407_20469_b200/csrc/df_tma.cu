@@ -826,13 +826,23 @@ __global__ void __launch_bounds__(tma::TH, 2) df_tma_kernel(const __grid_constan
             float sn, cs;
             sincosf(phi, &sn, &cs);
             const float2 x = have_x ? __ldcg(&xg_t[e]) : make_float2(0.f, 0.f);
-            o[Lsh.disc_f[e]] = cmulc(x, make_float2(cs, sn));
+            const int q = Lsh.disc_f[e];
+            const float2 u = cmulc(x, make_float2(cs, sn));
+            o[q] = Lsh.accumulate ? cadd(__ldcg(&o[q]), u) : u;   // ring-wise order (R15b): sum now, mean at the end of the ring
           }
           lb += cnt;
         }
         if (g == 0 && threadIdx.x == 0) a.cg_iters[size_t(slot) * a.n_leds + k] = iters;
       }
       team_sync(multi);                                    // O complete before the next LED reads it
+      if (Lsh.n_avg > 0) {                                 // df_order 1, end of a ring: bins solved by c LEDs hold a sum of c solutions
+        float2* o = o_t;
+        for (int i = int(g) * TH + threadIdx.x; i < Lsh.n_avg; i += int(G) * TH) {
+          const int q = __ldg(&Lsh.avg_f[i]);
+          o[q] = cscale(__ldcg(&o[q]), __ldg(&Lsh.avg_w[i]));
+        }
+        team_sync(multi);
+      }
     }
   }
   if (threadIdx.x == 0 && flop > 0.0) atomicAdd(a.work, (unsigned long long)(flop + 0.5));

@@ -118,12 +118,14 @@ bool build_geometry(const apic_params& p, HostTables& t, std::string& err) {
   if (p.n_bright < 3 || !p.k_bright) { err = "need >= 3 NA-matching LEDs"; return false; }
   if (p.n_dark < 0 || (p.n_dark > 0 && !p.k_dark)) { err = "k_dark missing"; return false; }
   if (p.n_zernike < 1 || p.n_zernike > 64 || !p.noll) { err = "n_zernike must be 1..64"; return false; }
-  if (p.kk_pad != 1) { err = "kk_pad: only 1 is implemented"; return false; }
+  if (p.kk_pad != 1 && p.kk_pad != 2) { err = "kk_pad must be 1 or 2"; return false; }
+  if (p.kk_pad * p.tile_n > 512) { err = "kk_pad 2 needs tile_n <= 256 (line transforms exist up to 512 points)"; return false; }
   if (p.refine_iters < 0 || p.refine_iters > 16) { err = "refine_iters must be 0..16"; return false; }
   if (p.df_iters < 1) { err = "df_iters must be >= 1"; return false; }
   if (p.bg_mode < 0 || p.bg_mode > 2) { err = "bg_mode must be 0, 1 or 2"; return false; }
   if (p.max_batch < 1) { err = "max_batch must be >= 1"; return false; }
   if (p.df_mode != 0 && p.df_mode != 3 && p.df_mode != 4) { err = "df_mode must be 0 (team kernel; reduced cyclic grids at N = 256), 3 (team kernel on the full N x N grid) or 4 (reduced grids with async-proxy staging)"; return false; }
+  if (p.df_order != 0 && p.df_order != 1) { err = "df_order must be 0 (sequential, R15) or 1 (ring-wise, R15b)"; return false; }
   if (!(p.df_team == 0 || p.df_team == 1 || p.df_team == 2 || p.df_team == 4 || p.df_team == 8)) {
     err = "df_team must be 0 (auto), 1, 2, 4 or 8"; return false;
   }
@@ -182,7 +184,9 @@ bool build_geometry(const apic_params& p, HostTables& t, std::string& err) {
   t.disc_off.assign(t.nb + 1, 0);
   t.bf_col0.resize(t.nb); t.bf_ncol.resize(t.nb);
   t.bf_map_off.assign(t.nb + 1, 0);
-  t.halfplane2.assign(size_t(t.nb) * n * n, 0);
+  const int M = p.kk_pad * n, hm = M / 2;              // grid of the KK step (R7): bins of the N grid are a subset of it
+  t.kk_n = M;
+  t.halfplane2.assign(size_t(t.nb) * M * M, 0);
   for (int i = 0; i < t.nb; ++i) {
     const double* kap = &t.kappa_b[2 * i];
     Mask m(n);
@@ -205,25 +209,25 @@ bool build_geometry(const apic_params& p, HostTables& t, std::string& err) {
       }
     t.disc_off[i + 1] = int32_t(t.disc_f.size());
     t.bf_col0[i] = c0; t.bf_ncol[i] = c1 - c0 + 1;
-    t.bf_map_off[i + 1] = t.bf_map_off[i] + n * t.bf_ncol[i];
+    t.bf_map_off[i + 1] = t.bf_map_off[i] + M * t.bf_ncol[i];
     t.bf_map.resize(t.bf_map_off[i + 1], -1);
     for (int iy = 0; iy < n; ++iy)
       for (int c = 0; c < t.bf_ncol[i]; ++c) {
-        int kx = c0 + c, ky = iy - h, fy = (ky + n) % n;
+        int kx = c0 + c, ky = iy - h, fy = (ky + M) % M;
         t.bf_map[size_t(t.bf_map_off[i]) + size_t(fy) * t.bf_ncol[i] + c] = entry_of[i][size_t(iy) * n + (kx + h)];
       }
-    // Eq. 5 weights, FFT order
+    // Eq. 5 weights on the KK grid, FFT order
     const double kn = std::hypot(kap[0], kap[1]);
-    uint8_t* w2 = &t.halfplane2[size_t(i) * n * n];
-    for (int ky = -h; ky < h; ++ky)
-      for (int kx = -h; kx < h; ++kx) {
+    uint8_t* w2 = &t.halfplane2[size_t(i) * M * M];
+    for (int ky = -hm; ky < hm; ++ky)
+      for (int kx = -hm; kx < hm; ++kx) {
         uint8_t v;
-        if (kx == -h || ky == -h) v = 1;
+        if (kx == -hm || ky == -hm) v = 1;
         else {
           double d = (kx * kap[0] + ky * kap[1]) / kn;
           v = (d < -kHalfplaneTau) ? 2 : ((d > kHalfplaneTau) ? 0 : 1);
         }
-        w2[fft_index(n, kx, ky)] = v;
+        w2[fft_index(M, kx, ky)] = v;
       }
     discs.push_back(std::move(m));
   }
@@ -289,8 +293,31 @@ bool build_geometry(const apic_params& p, HostTables& t, std::string& err) {
   for (int i = 0; i < t.nd; ++i)
     order.push_back({llround(std::hypot(t.kappa_d[2 * i], t.kappa_d[2 * i + 1]) / kOrderQuantum), i});
   std::stable_sort(order.begin(), order.end());
+  // df_order 1 (R15b): the LEDs of a ring (equal |kappa| key) all see the known set as it stands when the ring starts
+  const bool ring_wise = p.df_order == 1;
+  Mask base = known;                       // known set the current ring's LEDs are solved against
+  std::vector<int> cover(size_t(n) * n, 0);
+  int ring = -1;
+  long long ring_key = 0;
+  size_t ring_first = 0;                   // index in t.dark of the ring's first LED
+  auto close_ring = [&]() {
+    if (!ring_wise || t.dark.size() == ring_first) return;
+    DarkLed& last = t.dark.back();
+    for (int iy = 0; iy < n; ++iy)
+      for (int ix = 0; ix < n; ++ix) {
+        const int c = cover[size_t(iy) * n + ix];
+        if (c >= 2) { last.avg_f.push_back(fft_index(n, ix - h, iy - h)); last.avg_w.push_back(1.0f / float(c)); }
+      }
+    std::fill(cover.begin(), cover.end(), 0);
+  };
   for (auto& oi : order) {
     const int led = oi.second;
+    if (ring < 0 || oi.first != ring_key) {
+      close_ring();
+      ++ring; ring_key = oi.first; ring_first = t.dark.size();
+      base = known;
+    }
+    const Mask& ref = ring_wise ? base : known;
     const double* kap = &t.kappa_d[2 * led];
     Mask d(n), P(n), U(n);
     disc_mask(kap, d);
@@ -298,11 +325,12 @@ bool build_geometry(const apic_params& p, HostTables& t, std::string& err) {
     for (size_t q = 0; q < size_t(n) * n; ++q) {
       if (!d.v[q]) continue;
       ++nD;
-      if (known.v[q]) P.v[q] = 1; else { U.v[q] = 1; ++nU; }
+      if (ref.v[q]) P.v[q] = 1; else { U.v[q] = 1; ++nU; }
     }
     if (nU == 0) continue;
     DarkLed L;
     L.led = led; L.kappa[0] = kap[0]; L.kappa[1] = kap[1];
+    L.ring = ring; L.accumulate = ring_wise;
     L.unknown_fraction = double(nU) / nD;
     if (L.unknown_fraction > kMaxUnknown) {
       snprintf(buf, sizeof buf, "darkfield LED %d: unknown fraction %.3f > 0.42 (PAPER.md:201)", led, L.unknown_fraction);
@@ -392,9 +420,10 @@ bool build_geometry(const apic_params& p, HostTables& t, std::string& err) {
           if (Q.v[q]) L.qmask_m[pos(ix - h, iy - h)] = 1;
         }
     }
-    for (size_t q = 0; q < size_t(n) * n; ++q) known.v[q] |= U.v[q];
+    for (size_t q = 0; q < size_t(n) * n; ++q) { known.v[q] |= U.v[q]; cover[q] += U.v[q]; }
     t.dark.push_back(std::move(L));
   }
+  close_ring();
   t.n_known = known.count();
   {
     int x0 = n, x1 = -1, y0 = n, y1 = -1;

@@ -28,6 +28,12 @@ struct DarkLed {
   int q_row0 = 0, q_nrow = 0;
   std::vector<int32_t> disc_f; // [n_disc] FFT-order linear index of each disc entry
   std::vector<int32_t> u_row_off; // [u_nrow+1] first U entry of each row of the U bbox (U entries are row-major)
+  // ring-wise order (apic_params.df_order 1, reading R15b): the LED ADDS its solution to the object spectrum; the last
+  // LED of a ring carries the bins of the ring solved by c >= 2 LEDs, which are then scaled by 1 / c
+  int ring = 0;
+  bool accumulate = false;
+  std::vector<int32_t> avg_f;  // FFT-order linear index
+  std::vector<float> avg_w;    // 1 / c
   std::vector<float> zern;     // [n_disc][nz] Z_j(K + kappa)
   std::vector<int32_t> dmap;   // [N (fy)][d_ncol] -> disc entry or -1
   std::vector<int32_t> qmap;   // [N (fy)][q_ncol] -> equation index or -1
@@ -42,18 +48,19 @@ struct DarkLed {
 
 struct HostTables {
   int n = 0, u = 1, nb = 0, nd = 0, nz = 0;
+  int kk_n = 0;                             // grid of the KK step: kk_pad * N (R7); halfplane2 and bf_map live on it
   double radius = 0;
   std::vector<double> kappa_b, kappa_d;     // [nb][2], [nd][2] in bins
   std::vector<int> noll;
 
   // ---- NA-matching side
-  std::vector<uint8_t> halfplane2;          // [nb][N*N] FFT order, 2*w of Eq. 5 in {0,1,2}
+  std::vector<uint8_t> halfplane2;          // [nb][kk_n*kk_n] FFT order, 2*w of Eq. 5 in {0,1,2}
   std::vector<int32_t> disc_off;            // [nb+1] offsets into the flattened sub-spectrum vector
   std::vector<int32_t> disc_f;              // [disc_off[nb]] FFT-order index of each entry
   std::vector<float> disc_zern;             // [disc_off[nb]][nz]  Z_j(K+kappa_i) - Z_j(kappa_i)
   std::vector<int32_t> bf_col0, bf_ncol;    // [nb] centred kx range of each disc
   std::vector<int32_t> bf_map_off;          // [nb+1] offsets into bf_map
-  std::vector<int32_t> bf_map;              // per LED [N (fy)][ncol] -> flattened entry or -1
+  std::vector<int32_t> bf_map;              // per LED [kk_n (fy)][ncol] -> flattened entry or -1
 
   // ---- aberration system (Eq. 8-10)
   int n_pairs = 0;

@@ -129,7 +129,9 @@ void launch_zero_dead(const DevTables& t, const int32_t* status, int batch, floa
 }
 
 // ---------------------------------------------------------------------------------- S1-S2
-template <int N>
+// PADDED (kk_pad 2, R7): the image, Fourier-interpolated to the N = 2 x tile_n grid, is already in G (kk_pad_* below);
+// its real part is the input and the row is transformed in place.
+template <int N, bool PADDED>
 __global__ void __launch_bounds__(Strip<N>::THREADS, Strip<N>::MINB)
 kk_log_rowfft(DevTables t, ImgSrc src, const double* __restrict__ stats, float floor_rel,
               float2* __restrict__ G, const int32_t* __restrict__ live, const int32_t* __restrict__ live_count,
@@ -142,13 +144,16 @@ kk_log_rowfft(DevTables t, ImgSrc src, const double* __restrict__ stats, float f
   if (tile < 0) return;
   const int line = TH::line(), tt = TH::t(), y = blockIdx.x * S::LINES + line;
   const size_t ii = size_t(tile) * t.n_img + led;
-  const float mean = float(stats[(size_t(tile) * t.n_img + led) * 3] / double(N * N));
+  const float mean = float(stats[(size_t(tile) * t.n_img + led) * 3] / double(t.n * t.n));   // interpolation keeps the mean
   const float lo = floor_rel * mean;                                   // R6
+  float2* g = G + (size_t(slot) * t.nb + led) * (N * N) + y * N;
   float2 v[S::R];
 #pragma unroll
-  for (int r = 0; r < S::R; ++r) v[r] = make_float2(logf(fmaxf(img_load(src, ii, N * N, y * N + tt + S::TPL * r), lo)), 0.f);  // Re of Eq. 4
-  fft_regs<N, false>(v, sm + line * S::LS, tt, t.tw);
-  float2* g = G + (size_t(slot) * t.nb + led) * (N * N) + y * N;
+  for (int r = 0; r < S::R; ++r) {
+    const float x = PADDED ? g[tt + S::TPL * r].x : img_load(src, ii, N * N, y * N + tt + S::TPL * r);
+    v[r] = make_float2(logf(fmaxf(x, lo)), 0.f);                        // Re of Eq. 4
+  }
+  fft_regs<N, false>(v, sm + line * S::LS, tt, t.tw_kk);
 #pragma unroll
   for (int r = 0; r < S::R; ++r) g[tt + S::TPL * r] = v[r];
 }
@@ -167,12 +172,12 @@ kk_col_mask(DevTables t, float2* __restrict__ G, const int32_t* __restrict__ liv
   float2 v[S::R];
 #pragma unroll
   for (int r = 0; r < S::R; ++r) v[r] = g[(tt + S::TPL * r) * N];
-  fft_regs<N, false>(v, sm + line * S::LS, tt, t.tw);
+  fft_regs<N, false>(v, sm + line * S::LS, tt, t.tw_kk);
   const uint8_t* w2 = t.halfplane2 + size_t(led) * (N * N) + x;
   const float scale = 0.5f / float(N * N);                              // w = w2/2, and the 1/N^2 of F^-1
 #pragma unroll
   for (int r = 0; r < S::R; ++r) v[r] = cscale(v[r], float(__ldg(&w2[(tt + S::TPL * r) * N])) * scale);   // Eq. 5
-  fft_regs<N, true>(v, sm + line * S::LS, tt, t.tw);
+  fft_regs<N, true>(v, sm + line * S::LS, tt, t.tw_kk);
 #pragma unroll
   for (int r = 0; r < S::R; ++r) g[(tt + S::TPL * r) * N] = v[r];
 }
@@ -191,7 +196,7 @@ kk_row_exp(DevTables t, float2* __restrict__ G, const int32_t* __restrict__ live
   float2 v[S::R];
 #pragma unroll
   for (int r = 0; r < S::R; ++r) v[r] = g[tt + S::TPL * r];
-  fft_regs<N, true>(v, sm + line * S::LS, tt, t.tw);
+  fft_regs<N, true>(v, sm + line * S::LS, tt, t.tw_kk);
 #pragma unroll
   for (int r = 0; r < S::R; ++r) {
     const float a = expf(v[r].x);                                       // Eq. 6
@@ -199,7 +204,7 @@ kk_row_exp(DevTables t, float2* __restrict__ G, const int32_t* __restrict__ live
     sincosf(v[r].y, &sn, &cs);
     v[r] = make_float2(a * cs, a * sn);
   }
-  fft_regs<N, false>(v, sm + line * S::LS, tt, t.tw);
+  fft_regs<N, false>(v, sm + line * S::LS, tt, t.tw_kk);
 #pragma unroll
   for (int r = 0; r < S::R; ++r) g[tt + S::TPL * r] = v[r];
 }
@@ -223,7 +228,7 @@ kk_col_gather(DevTables t, const float2* __restrict__ G, float2* __restrict__ Sp
   float2 v[S::R];
 #pragma unroll
   for (int r = 0; r < S::R; ++r) v[r] = valid ? g[(tt + S::TPL * r) * N] : make_float2(0.f, 0.f);
-  fft_regs<N, false>(v, sm + line * S::LS, tt, t.tw);
+  fft_regs<N, false>(v, sm + line * S::LS, tt, t.tw_kk);
   if (!valid) return;
   const int32_t* map = t.bf_map + t.bf_map_off[led] + c;
   float2* s = Sp + size_t(slot) * t.disc_total;
@@ -235,22 +240,68 @@ kk_col_gather(DevTables t, const float2* __restrict__ G, float2* __restrict__ Sp
   }
 }
 
-template <int N>
+// ---------------------------------------------------------------------------------- kk_pad 2 (R7)
+// image -> complex N x N grid (the input of the N-grid transform)
+__global__ void __launch_bounds__(256) kk_pad_load(DevTables t, ImgSrc src, float2* __restrict__ KP,
+                                                   const int32_t* __restrict__ live, const int32_t* __restrict__ live_count,
+                                                   int chunk0) {
+  const int slot = blockIdx.z, led = blockIdx.y;
+  const int tile = resolve_tile_idx(live, live_count, chunk0, slot);
+  if (tile < 0) return;
+  const int nn = t.n * t.n;
+  const size_t ii = size_t(tile) * t.n_img + led;
+  float2* k = KP + (size_t(slot) * t.nb + led) * nn;
+  for (int q = blockIdx.x * 256 + threadIdx.x; q < nn; q += gridDim.x * 256) k[q] = make_float2(img_load(src, ii, nn, q), 0.f);
+}
+// spectrum on the N grid -> zero-padded spectrum on the M = 2N grid, / N^2, the sign-less Nyquist row and column of
+// the N grid split evenly between +N/2 and -N/2 (band-limited interpolation: values at the common points are kept)
+__global__ void __launch_bounds__(256) kk_pad_scatter(DevTables t, const float2* __restrict__ KP, float2* __restrict__ G,
+                                                      const int32_t* __restrict__ live_count, int chunk0) {
+  const int slot = blockIdx.z, led = blockIdx.y;
+  if (chunk0 + slot >= *live_count) return;
+  const int n = t.n, m = t.kk_n, h = n / 2;
+  const float2* k = KP + (size_t(slot) * t.nb + led) * (n * n);
+  float2* g = G + (size_t(slot) * t.nb + led) * (size_t(m) * m);
+  const float inv = 1.f / float(n * n);
+  for (int q = blockIdx.x * 256 + threadIdx.x; q < m * m; q += gridDim.x * 256) {
+    const int fy = q / m, fx = q - fy * m;
+    const int ky = fy < m / 2 ? fy : fy - m, kx = fx < m / 2 ? fx : fx - m;     // signed bins of the M grid
+    float w = inv;
+    if (ky < -h || ky > h || kx < -h || kx > h) w = 0.f;
+    if (ky == -h || ky == h) w *= 0.5f;
+    if (kx == -h || kx == h) w *= 0.5f;
+    float2 v = make_float2(0.f, 0.f);
+    if (w != 0.f) v = cscale(k[((ky + n) & (n - 1)) * n + ((kx + n) & (n - 1))], w);
+    g[q] = v;
+  }
+}
+
+template <int N, bool PADDED>
 static void launch_kk_n(const DevTables& t, const Workspace& w, const LaunchCtx& c, const ImgSrc& src,
                         const double* stats, float floor_rel) {
   using S = Strip<N>;
   constexpr int TH = S::THREADS;
   constexpr size_t SM = S::SMEM;
   if (!c.pd->attr_kk) {
-    cudaFuncSetAttribute(kk_log_rowfft<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
+    cudaFuncSetAttribute(kk_log_rowfft<N, PADDED>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
     cudaFuncSetAttribute(kk_col_mask<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
     cudaFuncSetAttribute(kk_row_exp<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
     cudaFuncSetAttribute(kk_col_gather<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(SM));
     c.pd->attr_kk = true;
   }
+  if (PADDED) {
+    // I -> F_N(I) -> zero-padded to the 2N grid -> F_2N^-1: the interpolated image (its real part is used)
+    ProfScope ps(c, CAT_KK_LOG_ROWFFT);
+    const int images = c.chunk_tiles * t.nb;
+    kk_pad_load<<<dim3(16, t.nb, c.chunk_tiles), 256, 0, c.stream>>>(t, src, w.KP, c.live, c.live_count, c.chunk0);
+    launch_fft2d(w.KP, t.n, images, false, t.tw, c.stream);
+    kk_pad_scatter<<<dim3(64, t.nb, c.chunk_tiles), 256, 0, c.stream>>>(t, w.KP, w.G, c.live_count, c.chunk0);
+    launch_fft2d(w.G, N, images, true, t.tw_kk, c.stream);
+    *c.launches += 5;                       // load, 2 + 2 transform passes, scatter (the scope above counted one)
+  }
   dim3 grid(N / S::LINES, t.nb, c.chunk_tiles);
   { ProfScope ps(c, CAT_KK_LOG_ROWFFT);
-    kk_log_rowfft<N><<<grid, TH, SM, c.stream>>>(t, src, stats, floor_rel, w.G, c.live, c.live_count, c.chunk0); }
+    kk_log_rowfft<N, PADDED><<<grid, TH, SM, c.stream>>>(t, src, stats, floor_rel, w.G, c.live, c.live_count, c.chunk0); }
   { ProfScope ps(c, CAT_KK_COL_MASK);
     kk_col_mask<N><<<grid, TH, SM, c.stream>>>(t, w.G, c.live_count, c.chunk0); }
   { ProfScope ps(c, CAT_KK_ROW_EXP);
@@ -262,11 +313,19 @@ static void launch_kk_n(const DevTables& t, const Workspace& w, const LaunchCtx&
 
 void launch_kk(const DevTables& t, const Workspace& w, const LaunchCtx& c, const ImgSrc& src, const double* stats,
                float floor_rel) {
-  switch (t.n) {
-    case 64: launch_kk_n<64>(t, w, c, src, stats, floor_rel); break;
-    case 128: launch_kk_n<128>(t, w, c, src, stats, floor_rel); break;
-    case 256: launch_kk_n<256>(t, w, c, src, stats, floor_rel); break;
-    case 512: launch_kk_n<512>(t, w, c, src, stats, floor_rel); break;
+  if (t.kk_n == t.n) {
+    switch (t.n) {
+      case 64: launch_kk_n<64, false>(t, w, c, src, stats, floor_rel); break;
+      case 128: launch_kk_n<128, false>(t, w, c, src, stats, floor_rel); break;
+      case 256: launch_kk_n<256, false>(t, w, c, src, stats, floor_rel); break;
+      case 512: launch_kk_n<512, false>(t, w, c, src, stats, floor_rel); break;
+    }
+  } else {                                   // kk_pad 2: the chain runs on the 2N grid
+    switch (t.kk_n) {
+      case 128: launch_kk_n<128, true>(t, w, c, src, stats, floor_rel); break;
+      case 256: launch_kk_n<256, true>(t, w, c, src, stats, floor_rel); break;
+      case 512: launch_kk_n<512, true>(t, w, c, src, stats, floor_rel); break;
+    }
   }
 }
 

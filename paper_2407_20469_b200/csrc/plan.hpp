@@ -13,15 +13,17 @@ namespace apic {
 struct DevTables {
   int n, u, nb, nd, nz, n_img;   // n_img = nb + nd
   const float2* tw;              // twiddle tables of fft_core.cuh (build_twiddles)
+  int kk_n;                      // grid of the KK step, kk_pad * N (R7)
+  const float2* tw_kk;           // twiddles of the kk_n-point line transform (= tw when kk_pad = 1)
   const float2* tw_xy;           // [5][256] twiddles of fft_xy.cuh for R1 = 6, 8, 10, 12, 16 (N = 256 only)
   // NA-matching side
-  const uint8_t* halfplane2;     // [nb][N*N] FFT order, 2*w of Eq. 5
+  const uint8_t* halfplane2;     // [nb][kk_n*kk_n] FFT order, 2*w of Eq. 5
   int disc_total;                // sum_i |D_i|
   const float* disc_zern;        // [disc_total][nz]  Z_j(K+kappa_i) - Z_j(kappa_i)
   const int32_t* bf_col0;        // [nb]
   const int32_t* bf_ncol;        // [nb]
   const int32_t* bf_map_off;     // [nb+1]
-  const int32_t* bf_map;         // per LED [N(fy)][ncol] -> flattened entry | -1
+  const int32_t* bf_map;         // per LED [kk_n(fy)][ncol] -> flattened entry | -1
   int bf_max_ncol;
   // aberration system
   int n_rows, n_grad;
@@ -58,6 +60,10 @@ struct DarkDev {
   const uint8_t* qmask_m;               // [my][mx] -> 1 on Q
   int u_strip_off[kMaxUStrips + 1];     // first U entry of each 16-row strip of the U rows (U entries are row-major)
   int u0m, q0m, d0m;                    // u_row0, q_row0, d_row0 mod my (first physical row on the reduced grid)
+  int accumulate;                       // df_order 1: the extension step adds to O instead of assigning
+  int n_avg;                            // last LED of a ring (df_order 1): bins solved by c >= 2 LEDs of the ring ...
+  const int32_t* avg_f;                 // ... their FFT-order index
+  const float* avg_w;                   // ... and 1 / c
 };
 
 constexpr int kGramRows = 512;          // rows per Gram partial (aberration kernels)
@@ -65,7 +71,8 @@ constexpr int kMaxZern = 64;
 
 struct Workspace {
   int chunk;               // tiles per pass
-  float2* G;               // [chunk][nb][N*N]   KK working grids
+  float2* G;               // [chunk][nb][kk_n*kk_n] KK working grids
+  float2* KP;              // [chunk][nb][N*N]   spectra of the intensities on the N grid (kk_pad 2 only)
   float2* S;               // [chunk][disc_total] sub-spectra on the discs (Eq. 7)
   float2* PR;              // [chunk][n_rows]    p = S_i conj S_l on the overlaps (Eq. 9)
   float* gram;             // [chunk][gram_parts][gram_entries]

@@ -137,6 +137,40 @@ def test_single_tile_configs(A, index):
     assert np.array_equal(Og != 0, np.fft.ifftshift(refs[0].known))
 
 
+def test_kk_pad_2_matches_oracle_and_removes_the_aliasing_floor(A):
+    """kk_pad = 2 (R7: the log of Eq. 5 is not band-limited; the image is Fourier-interpolated to the 2N grid and
+    the KK chain runs there).  Parity with the oracle at kk_pad 2 at the usual tolerances on configs 0, 1 and a
+    darkfield tile; and against the GROUND TRUTH on noise-free config 0 the stitched spectrum's error falls from
+    the 1e-4 aliasing floor of kk_pad 1 to fp32 rounding."""
+    from apic_synth import make_tile
+    from helpers import truth_object_spectrum
+    for cfg, tiles in ((get_config(0), [0]), (get_config(1), [0]), (get_config(2, tile_n=64, batch=2, grid=(2, 1)), [0, 1])):
+        stacks, _ = make_batch(cfg, tiles)
+        refs, geo = oracle_reconstruct(cfg, stacks, kk_pad=2)
+        plan, field, zern, pupil, status = gpu_reconstruct(A, cfg, stacks, kk_pad=2)
+        for b, ref in enumerate(refs):
+            check_tile(ref, field[b], zern[b], pupil[b], status[b], f"{cfg.name} kk_pad 2 tile {b}")
+        og = plan.debug_buffer(A.DBG_OBJECT_SPECTRUM, len(tiles)).cpu().numpy().reshape(len(tiles), cfg.tile_n, cfg.tile_n)
+        sets = O.darkfield_sets(geo)[0] if cfg.n_dark else None
+        for b, ref in enumerate(refs):
+            check_bands(geo, sets, og[b], ref, f"{cfg.name} kk_pad 2 tile {b}")
+    cfg = get_config(0)
+    _, truth = make_tile(cfg, 0, noise="none", keep_clean=True)
+    clean = truth.clean[None].astype(np.float32)
+    geo = O.Geometry(oracle_params(cfg))
+    target = truth_object_spectrum(cfg, truth, geo.radius)
+    bf = np.zeros((64, 64), bool)
+    for m in geo.disc_b:
+        bf |= m
+    err = {}
+    for pad in (1, 2):
+        plan, _, zern, _, _ = gpu_reconstruct(A, cfg, clean, kk_pad=pad)
+        og = np.fft.fftshift(plan.debug_buffer(A.DBG_OBJECT_SPECTRUM, 1).cpu().numpy()[0].reshape(64, 64))
+        err[pad] = rel_l2(og[bf], target[bf])
+    print("stitched spectrum vs ground truth, noise-free config 0:", err)
+    assert err[1] > 3e-5 and err[2] < 5e-6 and err[2] < 0.05 * err[1], err
+
+
 # ---------------------------------------------------------------------------------- config 2
 def test_config2_reduced_all_tiles_ragged_chunks(A):
     """64x64 variant of config 2 (8 + 16 LEDs, Poisson noise, 3x grid): every tile against the
@@ -537,6 +571,25 @@ def test_host_entry_pipelines_sub_batches_without_changing_bits(A):
         assert np.array_equal(field, ref[0]) and np.array_equal(zern, ref[1])
         assert np.array_equal(pupil, ref[2]) and np.array_equal(status, ref[3])
     assert np.array_equal(field[0], field[4]) and np.array_equal(field[1], field[69])
+
+
+@pytest.mark.parametrize("tile_n,df_mode", [(64, 0), (128, 0), (256, 0), (256, 4), (256, 3)])
+def test_ring_wise_darkfield_order_matches_the_oracles_second_reading(A, tile_n, df_mode):
+    """apic_params.df_order = 1 (reading R15b: every LED of a ring solved against the known set at the start of the
+    ring, overlaps averaged) against the oracle's dark_order='ring', through every darkfield kernel; and the two
+    readings differ from each other by far more than the parity bar, so the test cannot pass by accident."""
+    cfg = get_config(2, tile_n=tile_n, batch=2, grid=(2, 1)) if tile_n != 256 else get_config(2)
+    tiles = [0, 1] if tile_n != 256 else [5]
+    stacks, _ = make_batch(cfg, tiles)
+    refs, geo = oracle_reconstruct(cfg, stacks, dark_order="ring")
+    sets = O.darkfield_sets(geo)[0]
+    plan, field, zern, pupil, status = gpu_reconstruct(A, cfg, stacks, df_order=1, df_mode=df_mode)
+    og = plan.debug_buffer(A.DBG_OBJECT_SPECTRUM, len(tiles)).cpu().numpy().reshape(len(tiles), tile_n, tile_n)
+    _, field_seq, zern_seq, _, _ = gpu_reconstruct(A, cfg, stacks, df_mode=df_mode)
+    for b, ref in enumerate(refs):
+        check_tile(ref, field[b], zern[b], pupil[b], status[b], f"ring-wise N={tile_n} tile {b}")
+        check_bands(geo, sets, og[b], ref, f"ring-wise N={tile_n} tile {b}")
+        assert np.array_equal(zern[b], zern_seq[b]) and rel_l2(field[b], field_seq[b]) > 2 * FIELD_TOL
 
 
 def test_streaming_host_entry_keeps_two_batches_in_flight_without_changing_bits(A):

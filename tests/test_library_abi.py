@@ -127,6 +127,27 @@ def test_no_cpu_fallback(A):
         plan_from_config(A, cfg)
 
 
+def test_ring_wise_order_index_sets_match_the_oracle(A):
+    """df_order 1 (reading R15b): the library's |U|, |Q| per LED equal those of the oracle's dark_order='ring'
+    (independent code: run-length Minkowski differences here, all-pairs differences there), and its reduced grids
+    are alias-free for those sets."""
+    from oracle import apic_oracle as O
+    from helpers import oracle_params
+    for cfg in (get_config(2), get_config(2, tile_n=64, batch=1, grid=(1, 1))):
+        p, keep = _params(A, cfg, df_order=1)
+        _, dark = A.geometry_info(p)
+        sets, _ = O.darkfield_sets(O.Geometry(oracle_params(cfg, dark_order="ring")))
+        assert [(d.led, int(d.U.sum()), int(d.Q.sum())) for d in sets] == dark
+        seq = A.geometry_info(_params(A, cfg)[0])[1]
+        assert dark[0] == seq[0] and dark[8] == seq[8] and sum(d[1] for d in dark) > sum(d[1] for d in seq)
+        n = cfg.tile_n
+        for (mx, my), ds in zip(A.geometry_dark_grids(p), sets):
+            for m, axis in ((mx, 1), (my, 0)):
+                u, pp, q = (np.nonzero(mm.any(axis=1 - axis))[0] for mm in (ds.U, ds.P, ds.Q))
+                ext = max(abs(int(u.max() - pp.min() - (q.min() - n // 2))), abs(int(u.min() - pp.max() - (q.max() - n // 2))))
+                assert m > ext
+
+
 @pytest.mark.parametrize("index,tile_n", [(2, 256), (3, 256), (2, 64)])
 def test_reduced_darkfield_grids_are_alias_free(A, index, tile_n):
     """The library's per-LED cyclic grid (mx, my) for the CG mat-vecs of Eq. 13 must exceed, per axis,
