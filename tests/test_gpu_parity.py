@@ -141,7 +141,7 @@ def test_kk_pad_2_matches_oracle_and_removes_the_aliasing_floor(A):
     """kk_pad = 2 (R7: the log of Eq. 5 is not band-limited; the image is Fourier-interpolated to the 2N grid and
     the KK chain runs there).  Parity with the oracle at kk_pad 2 at the usual tolerances on configs 0, 1 and a
     darkfield tile; and against the GROUND TRUTH on noise-free config 0 the stitched spectrum's error falls from
-    the 1e-4 aliasing floor of kk_pad 1 to fp32 rounding."""
+    the aliasing floor of kk_pad 1 (3e-5 on this tile) to fp32 rounding (1e-7)."""
     from apic_synth import make_tile
     from helpers import truth_object_spectrum
     for cfg, tiles in ((get_config(0), [0]), (get_config(1), [0]), (get_config(2, tile_n=64, batch=2, grid=(2, 1)), [0, 1])):
@@ -168,7 +168,7 @@ def test_kk_pad_2_matches_oracle_and_removes_the_aliasing_floor(A):
         og = np.fft.fftshift(plan.debug_buffer(A.DBG_OBJECT_SPECTRUM, 1).cpu().numpy()[0].reshape(64, 64))
         err[pad] = rel_l2(og[bf], target[bf])
     print("stitched spectrum vs ground truth, noise-free config 0:", err)
-    assert err[1] > 3e-5 and err[2] < 5e-6 and err[2] < 0.05 * err[1], err
+    assert err[1] > 1e-5 and err[2] < 1e-6 and err[2] < 0.01 * err[1], err       # measured: 2.9e-5 -> 8.9e-8
 
 
 # ---------------------------------------------------------------------------------- config 2
