@@ -50,9 +50,11 @@ def parse_args():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (2 = default workload)")
     ap.add_argument("--tiles", type=int, default=0, help="tiles per step and per GPU (0 = the config's batch, capped at 64)")
     ap.add_argument("--chunk", type=int, default=0, help="apic_params.chunk_tiles (0 = library default)")
-    ap.add_argument("--df-mode", type=int, default=0, help="darkfield kernel: 0 team kernel (reduced grids at N=256), 3 team kernel on the full grid")
+    ap.add_argument("--df-mode", type=int, default=0, help="darkfield kernel: 0 team kernel (reduced grids at N=256), 3 team kernel on the full grid, "
+                    "4 reduced grids with async-proxy (TMA bulk copy) staging")
     ap.add_argument("--pass-tiles", type=int, default=592, help="config 4: tiles per apic_reconstruct_u16 call (a step)")
     ap.add_argument("--oracle-sample", type=int, default=0, help="config 4: live tiles compared with the fp64 oracle after the run")
+    ap.add_argument("--df-order", type=int, default=0, help="apic_params.df_order: 0 sequential (R15, the headline), 1 ring-wise (R15b)")
     ap.add_argument("--df-team", type=int, default=0, help="apic_params.df_team: CTAs per tile of the team kernel (0 = auto)")
     ap.add_argument("--df-tol", type=float, default=-1.0, help="CG tolerance (default: the library's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -450,7 +452,7 @@ def run_batch(ctx):
     host = np.concatenate([stacks] * reps)[:tiles]
     x = torch.from_numpy(host).cuda()
     popts = {"df_tol": args.df_tol} if args.df_tol > 0 else {}
-    plan = A.Plan(*plan_args(cfg), max_batch=tiles, chunk_tiles=args.chunk, df_mode=args.df_mode, df_team=args.df_team, **popts)
+    plan = A.Plan(*plan_args(cfg), max_batch=tiles, chunk_tiles=args.chunk, df_mode=args.df_mode, df_team=args.df_team, df_order=args.df_order, **popts)
     n, on, nz = cfg.tile_n, cfg.out_n, plan.nz
     out = (torch.empty((tiles, on, on), dtype=torch.complex64, device="cuda"),
            torch.empty((tiles, nz), dtype=torch.float32, device="cuda"),
@@ -566,7 +568,7 @@ def run_batch(ctx):
                 "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": workload_name(cfg, tiles), "tiles_per_step_per_gpu": tiles,
-                           "distinct_tiles": n_gen, "tiles_ok": n_ok,
+                           "distinct_tiles": n_gen, "tiles_ok": n_ok, "df_mode": args.df_mode, "df_order": args.df_order,
                            "tiles_per_s": world * args.steps * tiles / (ms / 1e3), "chunk_tiles": chunk,
                            "cache": "inputs larger than L2 "
                            f"({host.nbytes / 1e6:.0f} MB per step vs 126 MB L2)", "parallelism": f"tiles x{world}"},
