@@ -366,7 +366,7 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
   const size_t nn = size_t(n) * n;
   int chunk = p->chunk_tiles;
   if (chunk <= 0) {
-    if (n == 256 && (p->df_mode == 0 || p->df_mode == 4) && !h.dark.empty()) {
+    if (n == 256 && (p->df_mode == 0 || p->df_mode == 4 || p->df_mode == 5) && !h.dark.empty()) {
       // reduced-grid darkfield kernel: its CG working set is ~0.3 MB per tile (TM + p_M on grids of 15-20 k bins),
       // so the pass is sized for the kernel's scheduler instead: up to two tiles per SM (one CTA per tile)
       chunk = 2 * std::max(1, plan->pd.sms);
@@ -449,7 +449,10 @@ static int reconstruct_impl(apic_plan* plan, int zi, const ImgSrc& src, int batc
     launch_stitch(t, w, c);                                                                   // S7
     if (p.df_mode == 0 && t.n == 256)                                                         // S8-S10
       launch_darkfield_mgrid(t, plan->d_dark, n_dark_used, w, c, src, p.df_iters, p.df_tol, p.df_team);
-    else if (p.df_mode == 4 && t.n == 256)
+    else if (p.df_mode == 5 && t.n == 256) {
+      if (!launch_darkfield_wide(t, plan->d_dark, plan->dark.data(), n_dark_used, w, c, src, p.df_iters, p.df_tol, p.df_team, 0))
+        launch_darkfield_mgrid(t, plan->d_dark, n_dark_used, w, c, src, p.df_iters, p.df_tol, 0);
+    } else if (p.df_mode == 4 && t.n == 256)
       launch_darkfield_tma(t, plan->d_dark, plan->dark.data(), n_dark_used, w, c, src, p.df_iters, p.df_tol, p.df_team);
     else
       launch_darkfield_team(t, plan->d_dark, n_dark_used, w, c, src, p.df_iters, p.df_tol, p.df_team);
@@ -775,7 +778,7 @@ int apic_last_launch_count(const apic_plan* plan) { return plan ? plan->launches
 
 static const char* kCatNames[CAT_COUNT] = {
     "stats_status", "kk_log_rowfft", "kk_col_mask", "kk_row_exp", "kk_col_gather", "ab_pair_products", "ab_gram",
-    "ab_solve", "stitch", "out_rows", "out_cols", "pupil", "df_mgrid_kernel", "df_team_kernel", "df_tma_kernel"};
+    "ab_solve", "stitch", "out_rows", "out_cols", "pupil", "df_mgrid_kernel", "df_team_kernel", "df_tma_kernel", "df_wide_kernel"};
 
 int apic_profile_categories(void) { return CAT_COUNT; }
 const char* apic_profile_category_name(int cat) { return (cat >= 0 && cat < CAT_COUNT) ? kCatNames[cat] : ""; }

@@ -112,7 +112,7 @@ struct BatchState {
 // ------------------------------------------------------------------ per-kernel timing (apic_profile_*)
 enum KernelCat {
   CAT_STATS = 0, CAT_KK_LOG_ROWFFT, CAT_KK_COL_MASK, CAT_KK_ROW_EXP, CAT_KK_COL_GATHER, CAT_AB_PRODUCTS, CAT_AB_GRAM,
-  CAT_AB_SOLVE, CAT_STITCH, CAT_OUT_ROWS, CAT_OUT_COLS, CAT_PUPIL, CAT_DF_MGRID, CAT_DF_TEAM, CAT_DF_TMA, CAT_COUNT
+  CAT_AB_SOLVE, CAT_STITCH, CAT_OUT_ROWS, CAT_OUT_COLS, CAT_PUPIL, CAT_DF_MGRID, CAT_DF_TEAM, CAT_DF_TMA, CAT_DF_WIDE, CAT_COUNT
 };
 
 // Per-plan record of what has been set up on the plan's device (function attributes are per device, so the
@@ -188,6 +188,10 @@ void launch_darkfield_mgrid(const DevTables& t, const DarkDev* d_leds, int n_led
 // (df_tma.cu; N = 256, df_mode 4); h_leds = host copy of d_leds
 void launch_darkfield_tma(const DevTables& t, const DarkDev* d_leds, const DarkDev* h_leds, int n_leds, const Workspace& w,
                           const LaunchCtx& c, const ImgSrc& src, int df_iters, float df_tol, int team_size);
+// the same solver scheduled wide: NG strip groups of 256 threads per CTA at 64 registers, p_M strips parked in shared
+// memory, distributed CG vectors (df_wide.cu; N = 256, df_mode 5).  false: the configuration does not fit.
+bool launch_darkfield_wide(const DevTables& t, const DarkDev* d_leds, const DarkDev* h_leds, int n_leds, const Workspace& w,
+                           const LaunchCtx& c, const ImgSrc& src, int df_iters, float df_tol, int team_size, int groups);
 int launch_fft2d_xy(float2* d, int mx, int my, int batch, int mode, const float2* tw_xy, cudaStream_t s);
 // outputs
 void launch_output(const DevTables& t, const Workspace& w, const LaunchCtx& c, float* d_field, float* d_pupil);
