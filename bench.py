@@ -11,7 +11,7 @@ on (config 1 is a single tile, i.e. a latency case).  Prints ONE 
   value     output megapixels/s with the inputs resident in HBM (CUDA events, max over ranks)
   e2e       the same metric through apic_submit_host / apic_wait_host with pinned HOST buffers (H2D + D2H inside;
             two batches in flight), and through the blocking apic_reconstruct_host beside it
-  roofline  the dominant kernel (df_mgrid_kernel: the darkfield CG on reduced cyclic grids), timed live by CUDA
+  roofline  the dominant kernel (df_wide_kernel: the darkfield CG on reduced cyclic grids), timed live by CUDA
             events inside the library on the launching stream, against fp32 peaks MEASURED in this run
             (apic_measure_peak: FFMA and FADD register loops, shared-memory reads)
   cpu_baseline  the fp64 oracle, as it stands, on this box's host cores, on a bounded sample
@@ -50,8 +50,8 @@ def parse_args():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (2 = default workload)")
     ap.add_argument("--tiles", type=int, default=0, help="tiles per step and per GPU (0 = the config's batch, capped at 64)")
     ap.add_argument("--chunk", type=int, default=0, help="apic_params.chunk_tiles (0 = library default)")
-    ap.add_argument("--df-mode", type=int, default=0, help="darkfield kernel: 0 team kernel (reduced grids at N=256), 3 team kernel on the full grid, "
-                    "4 reduced grids with async-proxy (TMA bulk copy) staging")
+    ap.add_argument("--df-mode", type=int, default=0, help="darkfield kernel (apic.h): 0 default (df_wide.cu, 256-thread CTAs at 128 registers), "
+                    "3 full grid, 4 async-proxy staging, 5 1024-thread CTA pairs with the decimated CG loop, 6 the round-1 kernel")
     ap.add_argument("--pass-tiles", type=int, default=592, help="config 4: tiles per apic_reconstruct_u16 call (a step)")
     ap.add_argument("--oracle-sample", type=int, default=0, help="config 4: live tiles compared with the fp64 oracle after the run")
     ap.add_argument("--df-order", type=int, default=0, help="apic_params.df_order: 0 sequential (R15, the headline), 1 ring-wise (R15b)")
@@ -177,7 +177,7 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------ roofline helpers
-KERNEL_SOURCES = ("df_mgrid.cu", "df_tma.cu", "df_team.cu", "fft_xy.cuh", "fft_core.cuh")
+KERNEL_SOURCES = ("df_wide.cu", "df_mgrid.cu", "df_tma.cu", "df_team.cu", "fft_xy.cuh", "fft_core.cuh")
 
 
 def kernel_source_hash():

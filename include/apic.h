@@ -89,15 +89,26 @@ typedef struct {
                             0, whose working set is ~0.3 MB per tile), otherwise as many tiles as
                             keep the full-grid darkfield working set (1.7 N^2 complex64 per tile)
                             inside half of the device's L2 (queried), clamped to 8..512          */
-  int df_mode;           /* darkfield scheduler: 0 = team kernel (one launch per pass covers every
-                            darkfield LED; a cluster of df_team CTAs owns a tile and meets at
-                            cluster barriers between phases); at N = 256 it runs the CG mat-vecs
-                            on per-LED reduced cyclic grids.  3 = the team
-                            kernel on the full N x N grid (what other N run; kept at N = 256 as a
-                            cross-check of the reduced grids).  4 = the reduced-grid solver with
-                            strips staged into shared memory by the async proxy (cp.async.bulk +
-                            mbarrier, strip-major scratch) and the CG vectors distributed over the
-                            team (N = 256; other N fall back to the full-grid team kernel)      */
+  int df_mode;           /* darkfield scheduler.  Every mode runs one launch per pass that covers
+                            all darkfield LEDs; a thread-block cluster (team) owns a tile and
+                            meets at cluster barriers between phases.  At N = 256 modes 0, 4, 5, 6
+                            run the CG mat-vecs on per-LED reduced cyclic grids (DESIGN.md
+                            section 5); other N run mode 3 whatever is asked.
+                            0 = default: df_wide.cu in df_mgrid.cu's shape (teams of 256-thread
+                                CTAs, 128 registers, 2 CTAs per SM) with the p_M strips and Q
+                                masks parked in shared memory and the CG vectors distributed
+                                over the team.
+                            3 = the team kernel on the full N x N grid (cross-check of the
+                                reduced grids).
+                            4 = strips staged by the async proxy (cp.async.bulk + mbarrier,
+                                strip-major scratch), df_tma.cu.
+                            5 = pairs of 1024-thread CTAs at 64 registers (four strip groups per
+                                CTA); LEDs whose grid fits run the CG loop decimated 2 x 2 with
+                                the classes resident in shared memory (two cluster barriers per
+                                iteration), df_wide.cu.
+                            6 = df_mgrid.cu, the round-1 kernel (redundant CG vectors, plain
+                                loads).  Measured on config 2: 0 is the
+                                fastest, 4-6 are kept as named, parity-tested alternatives     */
   int df_team;           /* CTAs per tile, 1..8; 0 = chosen from the pass size (as many as the
                             pass leaves resident CTA slots for)                                 */
   int df_order;          /* order of the darkfield extension (PAPER.md:135 states none).  0 = one

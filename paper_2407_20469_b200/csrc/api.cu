@@ -366,7 +366,7 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
   const size_t nn = size_t(n) * n;
   int chunk = p->chunk_tiles;
   if (chunk <= 0) {
-    if (n == 256 && (p->df_mode == 0 || p->df_mode == 4 || p->df_mode == 5) && !h.dark.empty()) {
+    if (n == 256 && p->df_mode != 3 && !h.dark.empty()) {
       // reduced-grid darkfield kernel: its CG working set is ~0.3 MB per tile (TM + p_M on grids of 15-20 k bins),
       // so the pass is sized for the kernel's scheduler instead: up to two tiles per SM (one CTA per tile)
       chunk = 2 * std::max(1, plan->pd.sms);
@@ -447,12 +447,14 @@ static int reconstruct_impl(apic_plan* plan, int zi, const ImgSrc& src, int batc
     launch_kk(t, w, c, src, z.bs.stats, p.intensity_floor);                                   // S1-S5
     launch_aberration(t, w, c, p.refine_iters, d_zernike, d_status);                          // S6
     launch_stitch(t, w, c);                                                                   // S7
-    if (p.df_mode == 0 && t.n == 256)                                                         // S8-S10
-      launch_darkfield_mgrid(t, plan->d_dark, n_dark_used, w, c, src, p.df_iters, p.df_tol, p.df_team);
-    else if (p.df_mode == 5 && t.n == 256) {
-      if (!launch_darkfield_wide(t, plan->d_dark, plan->dark.data(), n_dark_used, w, c, src, p.df_iters, p.df_tol, p.df_team, 0))
+    if ((p.df_mode == 0 || p.df_mode == 5) && t.n == 256) {                                   // S8-S10
+      // df_wide.cu: mode 0 = 256-thread CTAs at 128 registers (groups 11), mode 5 = 1024-thread CTA pairs (groups 4)
+      if (!launch_darkfield_wide(t, plan->d_dark, plan->dark.data(), n_dark_used, w, c, src, p.df_iters, p.df_tol, p.df_team,
+                                 p.df_mode == 0 ? 11 : 4))
         launch_darkfield_mgrid(t, plan->d_dark, n_dark_used, w, c, src, p.df_iters, p.df_tol, 0);
-    } else if (p.df_mode == 4 && t.n == 256)
+    } else if (p.df_mode == 6 && t.n == 256)
+      launch_darkfield_mgrid(t, plan->d_dark, n_dark_used, w, c, src, p.df_iters, p.df_tol, p.df_team);
+    else if (p.df_mode == 4 && t.n == 256)
       launch_darkfield_tma(t, plan->d_dark, plan->dark.data(), n_dark_used, w, c, src, p.df_iters, p.df_tol, p.df_team);
     else
       launch_darkfield_team(t, plan->d_dark, n_dark_used, w, c, src, p.df_iters, p.df_tol, p.df_team);

@@ -18,10 +18,11 @@
 //     p is never held in registers across a transform (that is what kept df_mgrid.cu at 128 registers);
 //   * the CG vectors x, s, pdir, w are DISTRIBUTED over the slots: a slot keeps the entries of the U-row strips it
 //     transforms in phases A / E (U entries are row-major, so a strip's entries are one contiguous range).  The dot
-//     products of an iteration, <pdir, w>, <s, w>, <w, w>, <s, s>, are reduced together: every slot writes its four
-//     partial sums into every team member's shared memory (DSMEM) before the cluster barrier that ends phase E and all
-//     threads add the S partial sums in slot order, so alpha, beta and the convergence decision are bit-identical
-//     across the team.  ||s_new||^2 = ||s||^2 - 2 alpha <s, w> + alpha^2 <w, w> gives beta without a second reduction;
+//     products of an iteration, <pdir, w>, <s, w>, <w, w>, <s, s>, are reduced together: the owner of a 16-row strip of U
+//     writes the strip's four partial sums into every team member's shared memory (DSMEM) before the cluster barrier
+//     that ends phase E and all threads add the strips' sums in strip order, so alpha, beta and the convergence decision
+//     are bit-identical across the team AND independent of the team size (a batch gives the same bits however it is
+//     split into passes).  ||s_new||^2 = ||s||^2 - 2 alpha <s, w> + alpha^2 <w, w> gives beta without a second reduction;
 //     ||s||^2 itself is recomputed directly in the next iteration's reduction, so the recurrence never accumulates error.
 // The scratch grids TM / PF stay row-major in L2 as in df_mgrid.cu; the line transforms are fft_xy.cuh's X / Y pair and
 // fft_core.cuh's radix-16 pair with a group-local barrier.
@@ -602,51 +603,63 @@ __device__ __forceinline__ void for_own(const DarkDev& L, const Grp& g, F&& f) {
     lb += cnt;
   }
 }
-// Partial sums of this slot's entries -> slot [sigma] of every team member's totals (DSMEM).  init: s = pdir = w, x = 0.
+// Partial sums, one set per 16-row STRIP of U (not per slot, so that the association - and with it every bit of the
+// result - does not depend on the team size or the groups per CTA): the slot that owns strip st reduces the strip's
+// entries over its 256 threads in a fixed order and writes the four sums into totals[st] of every team member (DSMEM).
+// init: s = pdir = w, x = 0 first.
 __device__ __forceinline__ void cg_partials(const Ctx& c, const Grp& g, const Vecs& V, bool init, unsigned G) {
-  gsync(g);                                             // w of phase E complete
+  const DarkDev& L = *c.Lp();
+  const int n_u = (L.u_nrow + 15) >> 4;
   float2* ps = c.ps(g.grp);
-  float pw = 0.f, sw = 0.f, ww = 0.f, s2 = 0.f;
-  for_own(*c.Lp(), g, [&](int l, int e) {
-    const float2 w = V.w(l, e);
-    if (init) {
-      V.s(l, e) = w;
-      ps[l] = w;
-      V.x(l, e) = make_float2(0.f, 0.f);
-      s2 += w.x * w.x + w.y * w.y;
-    } else {
-      const float2 p = ps[l], s = V.s(l, e);
-      pw += p.x * w.x + p.y * w.y;                      // Re(conj(pdir) w) = ||C pdir||^2
-      sw += s.x * w.x + s.y * w.y;
-      ww += w.x * w.x + w.y * w.y;
-      s2 += s.x * s.x + s.y * s.y;
-    }
-  });
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    pw += __shfl_xor_sync(0xffffffffu, pw, o);
-    sw += __shfl_xor_sync(0xffffffffu, sw, o);
-    ww += __shfl_xor_sync(0xffffffffu, ww, o);
-    s2 += __shfl_xor_sync(0xffffffffu, s2, o);
-  }
   float4* red = c.red(g.grp);
-  if ((g.tid & 31) == 0) red[g.tid >> 5] = make_float4(pw, sw, ww, s2);
-  gsync(g);
-  if (g.tid < int(G)) {
-    float4 s = red[0];
-#pragma unroll
-    for (int i = 1; i < GT / 32; ++i) {
-      const float4 q = red[i];
-      s.x += q.x; s.y += q.y; s.z += q.z; s.w += q.w;
+  int lb = 0;
+  gsync(g);                                             // w of phase E complete
+  for (int st = g.sigma; st < n_u; st += g.S) {
+    const int e0 = L.u_strip_off[st], cnt = L.u_strip_off[st + 1] - e0;
+    float pw = 0.f, sw = 0.f, ww = 0.f, s2 = 0.f;
+    for (int j = g.tid; j < cnt; j += GT) {
+      const int l = lb + j, e = e0 + j;
+      const float2 w = V.w(l, e);
+      if (init) {
+        V.s(l, e) = w;
+        ps[l] = w;
+        V.x(l, e) = make_float2(0.f, 0.f);
+        s2 += w.x * w.x + w.y * w.y;
+      } else {
+        const float2 p = ps[l], s = V.s(l, e);
+        pw += p.x * w.x + p.y * w.y;                    // Re(conj(pdir) w) = ||C pdir||^2
+        sw += s.x * w.x + s.y * w.y;
+        ww += w.x * w.x + w.y * w.y;
+        s2 += s.x * s.x + s.y * s.y;
+      }
     }
-    unsigned remote;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(smem_u32(c.totals() + g.sigma)), "r"(unsigned(g.tid)));
-    asm volatile("st.shared::cluster.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(remote), "f"(s.x), "f"(s.y), "f"(s.z), "f"(s.w) : "memory");
+    lb += cnt;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      pw += __shfl_xor_sync(0xffffffffu, pw, o);
+      sw += __shfl_xor_sync(0xffffffffu, sw, o);
+      ww += __shfl_xor_sync(0xffffffffu, ww, o);
+      s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+    }
+    if ((g.tid & 31) == 0) red[g.tid >> 5] = make_float4(pw, sw, ww, s2);
+    gsync(g);
+    if (g.tid < int(G)) {
+      float4 s = red[0];
+#pragma unroll
+      for (int i = 1; i < GT / 32; ++i) {
+        const float4 q = red[i];
+        s.x += q.x; s.y += q.y; s.z += q.z; s.w += q.w;
+      }
+      unsigned remote;
+      asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(smem_u32(c.totals() + st)), "r"(unsigned(g.tid)));
+      asm volatile("st.shared::cluster.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(remote), "f"(s.x), "f"(s.y), "f"(s.z), "f"(s.w) : "memory");
+    }
+    gsync(g);                                           // red is reused by the slot's next strip
   }
 }
-__device__ __forceinline__ float4 cg_totals(const Ctx& c, int S) {   // after the team barrier
+__device__ __forceinline__ float4 cg_totals(const Ctx& c, int n_strips) {   // after the team barrier: strips in order
   float4 s = c.totals()[0];
-  for (int q = 1; q < S; ++q) {
+  for (int q = 1; q < n_strips; ++q) {
     const float4 r = c.totals()[q];
     s.x += r.x; s.y += r.y; s.z += r.z; s.w += r.w;
   }
@@ -1020,8 +1033,10 @@ __device__ __noinline__ int vr_cg(const Args& a, const Ctx c, unsigned cr, float
 }
 
 // ================================================================ the kernel
-template <int NG>
-__global__ void __launch_bounds__(NG * GT, 4 / NG) df_wide_kernel(const __grid_constant__ Args a) {
+// MINB = CTAs per SM the kernel is compiled for (register cap 64K / (NG * 256 * MINB)): NG * MINB = 4 is the 64-register
+// wide shape; NG = 1, MINB = 2 is df_mgrid.cu's shape (128 registers, 2 CTAs of 256 threads per SM) with this file's data path
+template <int NG, int MINB>
+__global__ void __launch_bounds__(NG * GT, MINB) df_wide_kernel(const __grid_constant__ Args a) {
   Ctx c;
   c.kex = a.kex; c.kpc = a.kpc; c.cap = a.cap; c.ng = NG;
   c.nvec = 4 - ((a.vec_global & 1) + (a.vec_global >> 1 & 1) + (a.vec_global >> 2 & 1));
@@ -1119,7 +1134,7 @@ __global__ void __launch_bounds__(NG * GT, 4 / NG) df_wide_kernel(const __grid_c
         }
         if (g.sigma == 0 && g.tid == 0) a.cg_iters[size_t(slot) * a.n_leds + k] = iters;
       } else {
-      const float gamma0 = cg_totals(c, g.S).w;
+      const float gamma0 = cg_totals(c, n_u).w;
       bool done = !(gamma0 > 0.f);
       // ---- CG on the normal equations
       while (!done && iters < a.max_iters) {
@@ -1148,7 +1163,7 @@ __global__ void __launch_bounds__(NG * GT, 4 / NG) df_wide_kernel(const __grid_c
         WD_MARK(11);
         flop += 2 * mine(n_u) * fx + 4 * mine(n_c) * fy + 2 * mine(n_q) * fx;
         ++iters;
-        const float4 tot = cg_totals(c, g.S);              // <pdir, w>, <s, w>, <w, w>, <s, s>
+        const float4 tot = cg_totals(c, n_u);              // <pdir, w>, <s, w>, <w, w>, <s, s>
         if (!(tot.x > 0.f)) break;
         const float gamma = tot.w, alpha = gamma / tot.x;
         const float gnew = fmaxf(gamma - 2.f * alpha * tot.y + alpha * alpha * tot.z, 0.f);   // ||s - alpha w||^2
@@ -1183,7 +1198,7 @@ __global__ void __launch_bounds__(NG * GT, 4 / NG) df_wide_kernel(const __grid_c
   if (g.tid == 0 && flop > 0.0) atomicAdd(a.work, (unsigned long long)(flop + 0.5));
 }
 
-template <int NG>
+template <int NG, int MINB>
 static bool launch_ng(const Args& a0, const DarkDev* h_leds, int n_leds, const LaunchCtx& c, int G, int sms) {
   Args a = a0;
   if (G < 1) G = 1;
@@ -1220,7 +1235,7 @@ static bool launch_ng(const Args& a0, const DarkDev* h_leds, int n_leds, const L
   if (dbg) fprintf(stderr, "df_wide: NG %d G %d kex %d kpc %d cap %d smem %zu\n", NG, G, a.kex, a.kpc, a.cap, smem);
   if (dbg) fprintf(stderr, "df_wide: vec_global %d\n", a.vec_global);
   if (smem > size_t(227 * 1024)) return false;
-  auto kern = df_wide_kernel<NG>;
+  auto kern = df_wide_kernel<NG, MINB>;
   cudaError_t e1 = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
   cudaError_t e2 = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
   if (dbg && (e1 != cudaSuccess || e2 != cudaSuccess)) fprintf(stderr, "df_wide: attr %s / %s\n", cudaGetErrorString(e1), cudaGetErrorString(e2));
@@ -1296,8 +1311,9 @@ bool launch_darkfield_wide(const DevTables& t, const DarkDev* d_leds, const Dark
   if (a.kex + a.kpc < 16 * S256::LS) a.kex = 16 * S256::LS - a.kpc;
   a.kex = (a.kex + 1) & ~1;
   const int sms = c.pd->sms;
-  int ng = groups > 0 ? groups : 4;
-  if (const char* e = getenv("APIC_DF_WIDE_NG")) ng = atoi(e);
+  int ng = groups > 0 ? groups : 4;   // 4, 2, 1: groups per CTA at 64 registers; 11: one group at 128 registers
+  if (groups != 11)
+    if (const char* e = getenv("APIC_DF_WIDE_NG")) ng = atoi(e);   // experiments with the shapes of mode 5
   int G = team_size;
   if (G <= 0) {
     // NG = 4: pairs of 1024-thread CTAs, one CTA per SM (the decimated CG loop needs exactly this shape; larger passes
@@ -1305,16 +1321,19 @@ bool launch_darkfield_wide(const DevTables& t, const DarkDev* d_leds, const Dark
     if (ng == 4) {
       G = 2;
     } else {
-      const int ctas = ng == 2 ? 2 * sms : 4 * sms;
+      // measured on config 2 with df_mgrid.cu's identical shape (ms per step): 32 tiles G = 8: 8.3; 56 tiles G = 5: 10.4;
+      // 64 tiles G = 4: 12.1; cluster sizes 6 and 7 place badly and are skipped
+      const int ctas = ng == 2 || ng == 11 ? 2 * sms : 4 * sms;
       G = 1;
-      for (int cand : {4, 2})
+      for (int cand : {8, 5, 4, 2})
         if (cand * c.chunk_tiles <= ctas) { G = cand; break; }
     }
   }
   switch (ng) {
-    case 4: return launch_ng<4>(a, h_leds, n_leds, c, G, sms);
-    case 2: return launch_ng<2>(a, h_leds, n_leds, c, G, sms);
-    default: return launch_ng<1>(a, h_leds, n_leds, c, G, sms);
+    case 4: return launch_ng<4, 1>(a, h_leds, n_leds, c, G, sms);
+    case 2: return launch_ng<2, 2>(a, h_leds, n_leds, c, G, sms);
+    case 11: return launch_ng<1, 2>(a, h_leds, n_leds, c, G, sms);   // 128 registers
+    default: return launch_ng<1, 4>(a, h_leds, n_leds, c, G, sms);
   }
 }
 

@@ -124,7 +124,7 @@ bool build_geometry(const apic_params& p, HostTables& t, std::string& err) {
   if (p.df_iters < 1) { err = "df_iters must be >= 1"; return false; }
   if (p.bg_mode < 0 || p.bg_mode > 2) { err = "bg_mode must be 0, 1 or 2"; return false; }
   if (p.max_batch < 1) { err = "max_batch must be >= 1"; return false; }
-  if (p.df_mode != 0 && p.df_mode != 3 && p.df_mode != 4 && p.df_mode != 5) { err = "df_mode must be 0 (team kernel; reduced cyclic grids at N = 256), 3 (team kernel on the full N x N grid), 4 (reduced grids with async-proxy staging) or 5 (reduced grids, wide scheduling)"; return false; }
+  if (p.df_mode != 0 && (p.df_mode < 3 || p.df_mode > 6)) { err = "df_mode must be 0 (default: reduced cyclic grids at N = 256), 3 (full N x N grid), 4 (async-proxy staging), 5 (1024-thread CTA pairs, decimated CG loop) or 6 (round-1 reduced-grid kernel)"; return false; }
   if (p.df_order != 0 && p.df_order != 1) { err = "df_order must be 0 (sequential, R15) or 1 (ring-wise, R15b)"; return false; }
   if (!(p.df_team == 0 || p.df_team == 1 || p.df_team == 2 || p.df_team == 4 || p.df_team == 8)) {
     err = "df_team must be 0 (auto), 1, 2, 4 or 8"; return false;

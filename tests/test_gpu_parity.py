@@ -271,19 +271,24 @@ def test_config2_full_size_bench_configuration(A):
     sample = [0, 9, 18, 27, 37, 45, 54, 63]
     refs, geo = oracle_reconstruct(cfg, stacks[sample])
     sets = O.darkfield_sets(geo)[0]
-    # df_mode 4: the same reduced-grid solver with strips staged by the async proxy (cp.async.bulk + mbarrier),
-    # strip-major scratch and the CG vectors distributed over the team; whole batch in the bench's launch
-    # configuration, the sampled tiles against the oracle band by band, every tile against df_mode 0
-    plan4, field4, zern4, pupil4, status4 = gpu_reconstruct(A, cfg, stacks, df_mode=4)
-    assert np.all(status4 == 0) and np.array_equal(zern4, zern)
-    og4 = plan4.debug_buffer(A.DBG_OBJECT_SPECTRUM, 64).cpu().numpy().reshape(64, 256, 256)
-    for ref, b in zip(refs, sample):
-        check_tile(ref, field4[b], zern4[b], pupil4[b], status4[b], f"cfg2 tile {b} (df_mode 4)")
-        check_bands(geo, sets, og4[b], ref, f"cfg2 tile {b} (df_mode 4)")
-    for b in tiles:
-        assert rel_l2(field4[b], field[b]) < 2e-5, b
-    _, field4b, _, _, _ = gpu_reconstruct(A, cfg, stacks, df_mode=4)
-    assert np.array_equal(field4, field4b)                              # bit-reproducible
+    # the named alternatives of the reduced-grid solver, each on the whole batch in the bench's launch configuration:
+    # the sampled tiles against the oracle band by band, every tile against the default, bit-reproducibility.
+    #   4: strips staged by the async proxy (cp.async.bulk + mbarrier), strip-major scratch (df_tma.cu)
+    #   5: pairs of 1024-thread CTAs at 64 registers, CG loop decimated 2 x 2 and resident in shared memory (df_wide.cu)
+    #   6: the round-1 kernel with redundant CG vectors (df_mgrid.cu)
+    for mode in (4, 5, 6):
+        plan_m, field_m, zern_m, pupil_m, status_m = gpu_reconstruct(A, cfg, stacks, df_mode=mode)
+        assert np.all(status_m == 0) and np.array_equal(zern_m, zern)
+        og_m = plan_m.debug_buffer(A.DBG_OBJECT_SPECTRUM, 64).cpu().numpy().reshape(64, 256, 256)
+        for ref, b in zip(refs, sample):
+            check_tile(ref, field_m[b], zern_m[b], pupil_m[b], status_m[b], f"cfg2 tile {b} (df_mode {mode})")
+            check_bands(geo, sets, og_m[b], ref, f"cfg2 tile {b} (df_mode {mode})")
+        for b in tiles:
+            assert rel_l2(field_m[b], field[b]) < 2e-5, (mode, b)
+        _, field_mb, _, _, _ = gpu_reconstruct(A, cfg, stacks, df_mode=mode)
+        assert np.array_equal(field_m, field_mb), mode                  # bit-reproducible
+    _, field_b, _, _, _ = gpu_reconstruct(A, cfg, stacks)
+    assert np.array_equal(field, field_b)                               # the default too
     og = plan.debug_buffer(A.DBG_OBJECT_SPECTRUM, 64).cpu().numpy().reshape(64, 256, 256)
     worst = {}
     for ref, b in zip(refs, sample):
@@ -573,7 +578,7 @@ def test_host_entry_pipelines_sub_batches_without_changing_bits(A):
     assert np.array_equal(field[0], field[4]) and np.array_equal(field[1], field[69])
 
 
-@pytest.mark.parametrize("tile_n,df_mode", [(64, 0), (128, 0), (256, 0), (256, 4), (256, 3)])
+@pytest.mark.parametrize("tile_n,df_mode", [(64, 0), (128, 0), (256, 0), (256, 4), (256, 5), (256, 6), (256, 3)])
 def test_ring_wise_darkfield_order_matches_the_oracles_second_reading(A, tile_n, df_mode):
     """apic_params.df_order = 1 (reading R15b: every LED of a ring solved against the known set at the start of the
     ring, overlaps averaged) against the oracle's dark_order='ring', through every darkfield kernel; and the two
