@@ -190,6 +190,15 @@ def kernel_source_hash():
     return h.hexdigest()[:16]
 
 
+def kernel_short_name(full):
+    """'void apic::wd::df_wide_kernel<1, 2>(apic::wd::Args)' -> 'df_wide_kernel'; '<unnamed>::peak_alu_kernel<0>(...)' -> 'peak_alu_kernel'."""
+    import re
+    s = full.replace("<unnamed>", "anon")
+    s = s.split("(")[0]
+    s = re.sub(r"<[^<>]*>", "", s)
+    return s.split("::")[-1].replace("void ", "").strip()
+
+
 def ncu_capture(kernel, workload):
     """Per-launch DRAM bytes and shared-memory wavefronts of `kernel` from the committed ncu --set full summary
     (profiles/r2_ncu_kernels.csv).  A row taken with other kernel sources than the ones in the tree is refused."""
@@ -239,7 +248,7 @@ def ncu_summary(args):
         if new:
             w.writeheader()
         for r in rows[2:]:
-            name = r[ix["Kernel Name"]].split("(")[0].split("::")[-1]
+            name = kernel_short_name(r[ix["Kernel Name"]])
             stall = {k: val(r, f"smsp__average_warps_issue_stalled_{k}_per_issue_active.ratio", False)
                      for k in ("barrier", "long_scoreboard", "short_scoreboard", "wait", "membar", "no_instruction", "not_selected",
                                "selected", "math_pipe_throttle", "mio_throttle", "lg_throttle", "branch_resolving", "dispatch_stall",
