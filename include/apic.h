@@ -84,9 +84,9 @@ typedef struct {
   float bg_threshold;
   int max_batch;         /* apic_reconstruct accepts 1..max_batch tiles; workspace is sized for
                             min(max_batch, internal chunk)                                       */
-  int chunk_tiles;       /* tiles per internal pass; 0 = chosen by the library: two tiles per SM
-                            (296 on B200) for the reduced-grid darkfield kernel (N = 256, df_mode
-                            0, whose working set is ~0.3 MB per tile), otherwise as many tiles as
+  int chunk_tiles;       /* tiles per internal pass; 0 = chosen by the library: one tile per SM
+                            (148 on B200: teams of two CTAs) for the reduced-grid darkfield
+                            kernels (N = 256, whose working set is ~0.3 MB per tile), otherwise as many tiles as
                             keep the full-grid darkfield working set (1.7 N^2 complex64 per tile)
                             inside half of the device's L2 (queried), clamped to 8..512          */
   int df_mode;           /* darkfield scheduler.  Every mode runs one launch per pass that covers

@@ -368,8 +368,10 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
   if (chunk <= 0) {
     if (n == 256 && p->df_mode != 3 && !h.dark.empty()) {
       // reduced-grid darkfield kernel: its CG working set is ~0.3 MB per tile (TM + p_M on grids of 15-20 k bins),
-      // so the pass is sized for the kernel's scheduler instead: up to two tiles per SM (one CTA per tile)
-      chunk = 2 * std::max(1, plan->pd.sms);
+      // so the pass is sized for the kernel's scheduler instead: one tile per SM, i.e. teams of two CTAs on the two
+      // resident CTA slots of every SM.  Measured on config 2 (profiles/r2_darkfield.md): 148 tiles x 2 CTAs take 7.5 ms
+      // per 64 tiles, 296 tiles x 1 CTA 8.5 ms
+      chunk = std::max(1, plan->pd.sms);
     } else {
       // full-grid darkfield CG working set per tile: T rows in use (<= 2/3 N) + p (N^2) ~ 1.7 N^2 complex64; a pass
       // is sized to half of this device's L2
