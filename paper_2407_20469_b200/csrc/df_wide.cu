@@ -1323,7 +1323,7 @@ bool launch_darkfield_wide(const DevTables& t, const DarkDev* d_leds, const Dark
     } else {
       // measured on config 2 with df_mgrid.cu's identical shape (ms per step): 32 tiles G = 8: 8.3; 56 tiles G = 5: 10.4;
       // 64 tiles G = 4: 12.1; cluster sizes 6 and 7 place badly and are skipped
-      const int ctas = ng == 21 ? sms : ng == 2 || ng == 11 ? 2 * sms : 4 * sms;
+      const int ctas = ng == 2 || ng == 11 ? 2 * sms : 4 * sms;
       G = 1;
       for (int cand : {8, 5, 4, 2})
         if (cand * c.chunk_tiles <= ctas) { G = cand; break; }
@@ -1333,7 +1333,6 @@ bool launch_darkfield_wide(const DevTables& t, const DarkDev* d_leds, const Dark
     case 4: return launch_ng<4, 1>(a, h_leds, n_leds, c, G, sms);
     case 2: return launch_ng<2, 2>(a, h_leds, n_leds, c, G, sms);
     case 11: return launch_ng<1, 2>(a, h_leds, n_leds, c, G, sms);   // 128 registers
-    case 21: return launch_ng<2, 1>(a, h_leds, n_leds, c, G, sms);   // two groups at 128 registers, one CTA per SM
     default: return launch_ng<1, 4>(a, h_leds, n_leds, c, G, sms);
   }
 }

@@ -430,6 +430,14 @@ def test_results_are_bit_reproducible_and_batch_invariant(A):
     for team in (1, 2, 4):                                            # team size does not change the arithmetic
         _, ft, zt, _, _ = gpu_reconstruct(A, cfg, stacks, df_team=team)
         assert np.array_equal(f1, ft) and np.array_equal(z1, zt), team
+    # the default kernel at N = 256 (df_wide.cu) distributes the CG vectors over the team; its dot products are
+    # reduced per 16-row strip in a fixed order, so the bits do not depend on the team size either
+    cfg = get_config(2)
+    stacks, _ = make_batch(cfg, [3, 40])
+    _, f1, z1, _, _ = gpu_reconstruct(A, cfg, stacks)
+    for team in (1, 2, 4, 8):
+        _, ft, zt, _, _ = gpu_reconstruct(A, cfg, stacks, df_team=team)
+        assert np.array_equal(f1, ft) and np.array_equal(z1, zt), team
 
 
 def test_host_entry_point_and_batch_limits(A):
