@@ -36,6 +36,8 @@ struct WsSet {
   BatchState bs{};
   int32_t* h_live_count = nullptr;   // pinned
   bool ready = false;
+  cudaStream_t aux = nullptr;        // KK sub-passes alternate between the caller's stream and this one
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
 };
 
 struct apic_plan {
@@ -439,13 +441,19 @@ static int reconstruct_impl(apic_plan* plan, int zi, const ImgSrc& src, int batc
     if (!cuda_ok(cudaStreamSynchronize(s), "background pass")) return APIC_ECUDA;
     n_live = *z.h_live_count;
   }
+  if (!z.aux) {
+    if (!cuda_ok(cudaStreamCreateWithFlags(&z.aux, cudaStreamNonBlocking), "cudaStreamCreate") ||
+        !cuda_ok(cudaEventCreateWithFlags(&z.ev_fork, cudaEventDisableTiming), "cudaEventCreate") ||
+        !cuda_ok(cudaEventCreateWithFlags(&z.ev_join, cudaEventDisableTiming), "cudaEventCreate"))
+      return APIC_ECUDA;
+  }
   const int n_dark_used = int(plan->dark.size());
   // balanced passes: ceil(n_live / chunk) passes of (almost) equal size
   const int n_pass = (n_live + w.chunk - 1) / w.chunk;
   const int per_pass = n_pass ? (n_live + n_pass - 1) / n_pass : 0;
   for (int c0 = 0; c0 < n_live; c0 += per_pass) {
     LaunchCtx c{s, &plan->launches, &plan->prof, z.bs.live, z.bs.live_count, c0, std::min(per_pass, n_live - c0),
-                &plan->pd};
+                &plan->pd, z.aux, z.ev_fork, z.ev_join};
     launch_kk(t, w, c, src, z.bs.stats, p.intensity_floor);                                   // S1-S5
     launch_aberration(t, w, c, p.refine_iters, d_zernike, d_status);                          // S6
     launch_stitch(t, w, c);                                                                   // S7

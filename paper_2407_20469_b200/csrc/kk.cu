@@ -8,6 +8,8 @@
 //   kk_col_mask   : column FFT, w, column IFFT [y][kx] -> [ky][kx] -> [y][kx]
 //   kk_row_exp    : row IFFT, exp, row FFT     [y][kx] -> [y][x]   -> [y][kx]
 //   kk_col_gather : column FFT on the disc's columns only, gather D_i
+#include <algorithm>
+
 #include "fft_core.cuh"
 #include "plan.hpp"
 
@@ -299,16 +301,47 @@ static void launch_kk_n(const DevTables& t, const Workspace& w, const LaunchCtx&
     launch_fft2d(w.G, N, images, true, t.tw_kk, c.stream);
     *c.launches += 5;                       // load, 2 + 2 transform passes, scatter (the scope above counted one)
   }
-  dim3 grid(N / S::LINES, t.nb, c.chunk_tiles);
-  { ProfScope ps(c, CAT_KK_LOG_ROWFFT);
-    kk_log_rowfft<N, PADDED><<<grid, TH, SM, c.stream>>>(t, src, stats, floor_rel, w.G, c.live, c.live_count, c.chunk0); }
-  { ProfScope ps(c, CAT_KK_COL_MASK);
-    kk_col_mask<N><<<grid, TH, SM, c.stream>>>(t, w.G, c.live_count, c.chunk0); }
-  { ProfScope ps(c, CAT_KK_ROW_EXP);
-    kk_row_exp<N><<<grid, TH, SM, c.stream>>>(t, w.G, c.live_count, c.chunk0); }
-  dim3 grid4((t.bf_max_ncol + S::LINES - 1) / S::LINES, t.nb, c.chunk_tiles);
-  { ProfScope ps(c, CAT_KK_COL_GATHER);
-    kk_col_gather<N><<<grid4, TH, SM, c.stream>>>(t, w.G, w.S, c.live_count, c.chunk0); }
+  // The four strip kernels alternate between row and column strips, so every kernel boundary is a transposition
+  // through memory.  The grids of a whole pass (nb N^2 complex64 per tile: 268 MB for 64 tiles of config 2) do not fit
+  // the L2, so the pass is cut into sub-passes whose grids do (two sub-passes in flight on two streams, so that the
+  // launch tails of one overlap the other): only the images in and the sub-spectra out touch HBM.
+  const size_t per_tile = size_t(t.nb) * N * N * sizeof(float2);
+  int sub = c.chunk_tiles;
+  if (!PADDED && c.aux && per_tile * c.chunk_tiles > size_t(c.pd->l2_bytes) * 4 / 10) {
+    sub = std::max(1, int(size_t(c.pd->l2_bytes) * 4 / 10 / per_tile));
+    const int n_sub = (c.chunk_tiles + sub - 1) / sub;
+    sub = (c.chunk_tiles + n_sub - 1) / n_sub;            // balanced
+  }
+  const bool split = sub < c.chunk_tiles;
+  if (split) {
+    cudaEventRecord(c.ev_fork, c.stream);
+    cudaStreamWaitEvent(c.aux, c.ev_fork, 0);
+  }
+  int k = 0;
+  for (int s0 = 0; s0 < c.chunk_tiles; s0 += sub, ++k) {
+    const int ns = std::min(sub, c.chunk_tiles - s0);
+    LaunchCtx cs = c;
+    cs.stream = (split && (k & 1)) ? c.aux : c.stream;
+    // a sub-pass reuses the grid region of the sub-pass two before it (same stream, so ordered): the dead grids are
+    // overwritten while they still sit in L2 instead of being written back to HBM
+    float2* G = w.G + size_t(split ? (k & 1) * sub : s0) * t.nb * N * N;
+    float2* Sp = w.S + size_t(s0) * t.disc_total;
+    const int ch0 = c.chunk0 + s0;
+    dim3 grid(N / S::LINES, t.nb, ns);
+    { ProfScope ps(cs, CAT_KK_LOG_ROWFFT);
+      kk_log_rowfft<N, PADDED><<<grid, TH, SM, cs.stream>>>(t, src, stats, floor_rel, G, c.live, c.live_count, ch0); }
+    { ProfScope ps(cs, CAT_KK_COL_MASK);
+      kk_col_mask<N><<<grid, TH, SM, cs.stream>>>(t, G, c.live_count, ch0); }
+    { ProfScope ps(cs, CAT_KK_ROW_EXP);
+      kk_row_exp<N><<<grid, TH, SM, cs.stream>>>(t, G, c.live_count, ch0); }
+    dim3 grid4((t.bf_max_ncol + S::LINES - 1) / S::LINES, t.nb, ns);
+    { ProfScope ps(cs, CAT_KK_COL_GATHER);
+      kk_col_gather<N><<<grid4, TH, SM, cs.stream>>>(t, G, Sp, c.live_count, ch0); }
+  }
+  if (split) {
+    cudaEventRecord(c.ev_join, c.aux);
+    cudaStreamWaitEvent(c.stream, c.ev_join, 0);
+  }
 }
 
 void launch_kk(const DevTables& t, const Workspace& w, const LaunchCtx& c, const ImgSrc& src, const double* stats,

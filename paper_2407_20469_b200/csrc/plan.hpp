@@ -143,6 +143,8 @@ struct LaunchCtx {
   int chunk0;              // first live-list position of this chunk
   int chunk_tiles;         // grid size in tiles (CTAs beyond live_count exit)
   PlanDevice* pd;          // per-plan device state (attribute set-up flags, SM count)
+  cudaStream_t aux = nullptr;          // second stream of this workspace set (KK sub-passes alternate between the two) ...
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;   // ... and the events that fork it from / join it into `stream`
 };
 
 // stats / status (batch-level)
