@@ -83,16 +83,34 @@ __global__ void __launch_bounds__(256) ab_gram(DevTables t, const float2* __rest
     }
   }
   __syncthreads();
+  // Gram entries of the 512 rows: the two halves of the CTA take 256 rows each (four independent accumulators per
+  // thread instead of one 512-long dependent chain), the upper half hands its sums over through shared memory.
   float* out = gram + (size_t(slot) * gram_parts + part) * gram_entries;
-  for (int e = threadIdx.x; e < gram_entries; e += 256) {
-    // decode e -> (j <= k) in row-major upper-triangle order
-    int j = 0, rem = e;
-    while (rem >= ncol - j) { rem -= ncol - j; ++j; }
-    const int k = j + rem;
+  float* hand = smf + kGramRows * ld;                    // [gram_entries]
+  const int half = threadIdx.x >> 7, r0 = half * (kGramRows / 2);
+  for (int e0 = 0; e0 < gram_entries; e0 += 128) {
+    const int e = e0 + (threadIdx.x & 127);
     float acc = 0.f;
-#pragma unroll 8
-    for (int lr = 0; lr < kGramRows; ++lr) acc += smf[lr * ld + j] * smf[lr * ld + k];
-    out[e] = acc;
+    if (e < gram_entries) {
+      // decode e -> (j <= k) in row-major upper-triangle order
+      int j = 0, rem = e;
+      while (rem >= ncol - j) { rem -= ncol - j; ++j; }
+      const int k = j + rem;
+      const float* a = smf + r0 * ld + j;
+      const float* b = smf + r0 * ld + k;
+      float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+#pragma unroll 4
+      for (int lr = 0; lr < kGramRows / 2; lr += 4) {
+        a0 += a[(lr + 0) * ld] * b[(lr + 0) * ld];
+        a1 += a[(lr + 1) * ld] * b[(lr + 1) * ld];
+        a2 += a[(lr + 2) * ld] * b[(lr + 2) * ld];
+        a3 += a[(lr + 3) * ld] * b[(lr + 3) * ld];
+      }
+      acc = (a0 + a1) + (a2 + a3);
+      if (half) hand[e] = acc;
+    }
+    __syncthreads();
+    if (!half && e < gram_entries) out[e] = acc + hand[e];
   }
 }
 
@@ -181,7 +199,7 @@ __global__ void __launch_bounds__(128) ab_solve(DevTables t, const float* __rest
 
 void launch_aberration(const DevTables& t, const Workspace& w, const LaunchCtx& c, int refine_iters,
                        float* d_zernike, int32_t* d_status) {
-  const size_t sm = size_t(kGramRows) * ((t.nz + 2) | 1) * sizeof(float);
+  const size_t sm = (size_t(kGramRows) * ((t.nz + 2) | 1) + size_t(w.gram_entries)) * sizeof(float);
   if (!c.pd->attr_ab) {
     cudaFuncSetAttribute(ab_gram<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(ab_gram<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
