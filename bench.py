@@ -64,6 +64,8 @@ def parse_args():
                     "to profiles/r2_ncu_kernels.csv (with --commit and --workload)")
     ap.add_argument("--commit", default="", help="--ncu-summary: the commit the capture was taken at")
     ap.add_argument("--workload", default="", help="--ncu-summary: workload tag, e.g. cfg2_64tiles")
+    ap.add_argument("--reassemble", action="store_true", help="no reconstruction: time apic_reassemble (within-FOV reassembly of "
+                    "5 x 5 tiles of 768 x 768 output pixels with 10 %% overlap) against the HBM roofline")
     ap.add_argument("--dense-probe", action="store_true", help="no run of the library: time the dense route of the darkfield "
                     "step (G = C^H C with the library GEMM on tensor cores) for the shapes of config 2")
     return ap.parse_args()
@@ -323,6 +325,45 @@ def dense_probe():
                       "note": "8 LEDs per ring; building C and the right-hand sides not included"}), flush=True)
 
 
+def reassemble_bench(args):
+    """apic_reassemble on FOVs shaped like the paper's (5 x 5 patches per FOV) with config 4's 10 % overlap:
+    25 tiles of 768 x 768 complex64 in, one 3536 x 3536 FOV out per call; several FOVs so that the data exceeds the L2."""
+    import torch
+    import paper_2407_20469_b200 as A
+    torch.cuda.set_device(0)
+    ty = tx = 5
+    t, ov, n_fov = 768, 76, 4
+    g = torch.Generator(device="cuda").manual_seed(1)
+    tiles = [torch.view_as_complex(torch.rand((ty, tx, t, t, 2), device="cuda", generator=g) - 0.5).contiguous() for _ in range(n_fov)]
+    h = ty * (t - ov) + ov
+    outs = [torch.empty((h, h), dtype=torch.complex64, device="cuda") for _ in range(n_fov)]
+    steps = max(args.steps or 20, 1)
+    for w in range(max(args.warmup, 3)):
+        for f, o in zip(tiles, outs):
+            A.reassemble(f, ov, True, out=o)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for k in range(steps):
+        for f, o in zip(tiles, outs):
+            A.reassemble(f, ov, True, out=o)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / (steps * n_fov)
+    overlap_bytes = (ty * (tx - 1) + tx * (ty - 1)) * 2 * ov * t * 8          # the correlation pass reads every overlap twice
+    algo = ty * tx * t * t * 8 + h * h * 8 + overlap_bytes
+    peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))) if os.path.exists(os.path.join(ROOT, "MEASURED_PEAKS.json")) else {}
+    peak = peaks.get("hbm_gbs", 6650.0)
+    gbs = algo / (ms * 1e-3) / 1e9
+    print(json.dumps({"metric": "reassembled FOV megapixels/sec", "value": h * h / 1e6 / (ms * 1e-3), "unit": "Mpx/s",
+                      "ms_per_fov": ms, "steps": steps, "fovs_per_step": n_fov, "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": f"{ty} x {tx} tiles of {t} x {t} complex64, overlap {ov}, FOV {h} x {h}, align on; "
+                                             f"{n_fov} FOVs per step ({n_fov * algo / 1e6:.0f} MB > L2)"},
+                      "roofline": {"bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
+                                   "algorithmic_bytes_per_fov": algo, "traffic": None,
+                                   "peak_note": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback 6650 GB/s"}}), flush=True)
+
+
 def measured_peaks(A, torch, sm_mhz_max, sms):
     """fp32 FFMA / FADD rates and shared-memory read bandwidth measured on this device now; the derived figures
     (unit counts x clock) beside them."""
@@ -341,6 +382,9 @@ def main():
     args = parse_args()
     if args.ncu_summary:
         ncu_summary(args)
+        return
+    if args.reassemble:
+        reassemble_bench(args)
         return
     if args.dense_probe:
         dense_probe()

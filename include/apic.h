@@ -221,6 +221,21 @@ int apic_submit_host_u16(apic_plan* plan, int slot, const uint16_t* h_raw, const
                          float* h_field, float* h_zernike, float* h_pupil, int32_t* h_status);
 int apic_wait_host(apic_plan* plan, int slot);
 
+/* Within-FOV reassembly of overlapping reconstructed tiles ("individually
+ * reconstructed and then stitched together", "the overlapping regions were blended"; the blend and the
+ * global-phase treatment are readings B6-B8 of DESIGN.md).  d_fields: [tiles_y][tiles_x][tile_px][tile_px] complex64
+ * (the fields apic_reconstruct returns, tile_px = upsample * tile_n), tiles on a regular grid sharing `overlap` pixels
+ * with each neighbour, 0 <= 2 overlap <= tile_px.  d_fov: [H][W] complex64, H = tiles_y (tile_px - overlap) + overlap
+ * (W likewise): the separable linear blend of the tiles, each multiplied by its unit factor d_factors[tile] (complex64,
+ * written by the call).  align != 0: the factors bring every tile to the global phase of tile (0, 0) in raster order
+ * through the correlation of its overlaps with the left / upper neighbour (tiles come out of apic_reconstruct with
+ * their own DC real-positive, so neighbours differ by a unit factor); align == 0: all factors 1.  d_work: device
+ * scratch of apic_reassemble_work_bytes(tiles_y, tiles_x) bytes.  All pointers are DEVICE pointers owned by the caller;
+ * the call only enqueues three kernels on cuda_stream.  Stateless (no plan).  Returns APIC_EINVAL on bad geometry. */
+size_t apic_reassemble_work_bytes(int tiles_y, int tiles_x);
+int apic_reassemble(const float* d_fields, int tiles_y, int tiles_x, int tile_px, int overlap, int align, float* d_fov,
+                    float* d_factors, void* d_work, void* cuda_stream);
+
 /* Stage-level access for parity tests (device pointers, valid after apic_reconstruct on the
  * same stream, for the tiles of the LAST internal chunk; tile index is chunk-local):
  *   APIC_DBG_SUBSPECTRA: [chunk][sum_i |D_i|] complex64, S_hat_i on D_i (Eq. 7), LED-major, bins

@@ -25,7 +25,8 @@ EXPORTS = ("apic_params_default", "apic_plan_create", "apic_plan_destroy", "apic
            "apic_submit_host", "apic_submit_host_u16", "apic_wait_host",
            "apic_debug_buffer", "apic_debug_copy", "apic_fft2d", "apic_fft2d_xy", "apic_last_launch_count", "apic_strerror",
            "apic_last_cuda_error", "apic_version", "apic_profile_categories", "apic_profile_category_name",
-           "apic_profile_begin", "apic_profile_end", "apic_profile_work", "apic_measure_peak")
+           "apic_profile_begin", "apic_profile_end", "apic_profile_work", "apic_measure_peak", "apic_reassemble",
+           "apic_reassemble_work_bytes")
 
 
 class ApicError(RuntimeError):
@@ -100,6 +101,10 @@ def load() -> C.CDLL:
                                      C.POINTER(C.c_longlong)]
     lib.apic_profile_work.argtypes = [C.c_void_p, C.POINTER(C.c_ulonglong)]
     lib.apic_measure_peak.argtypes = [C.c_int, C.POINTER(C.c_double), C.c_void_p]
+    lib.apic_reassemble_work_bytes.argtypes = [C.c_int, C.c_int]
+    lib.apic_reassemble_work_bytes.restype = C.c_size_t
+    lib.apic_reassemble.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
+                                    C.c_void_p]
     _lib = lib
     return lib
 
@@ -340,6 +345,30 @@ def measure_peak(what: int) -> float:
     _check(load().apic_measure_peak(int(what), C.byref(v), C.c_void_p(torch.cuda.current_stream().cuda_stream)),
            "apic_measure_peak")
     return float(v.value)
+
+
+def reassemble(fields, overlap: int, align: bool = True, out=None):
+    """apic_reassemble: fields = complex64 CUDA tensor [tiles_y][tiles_x][T][T] (reconstructed tiles on a regular grid
+    sharing `overlap` pixels).  Returns (fov complex64 [H][W], factors complex64 [tiles_y][tiles_x])."""
+    import torch
+    if not (fields.is_cuda and fields.dtype == torch.complex64 and fields.is_contiguous() and fields.dim() == 4
+            and fields.shape[2] == fields.shape[3]):
+        raise ApicError("fields must be a contiguous complex64 CUDA tensor [tiles_y][tiles_x][T][T]")
+    ty, tx, t = int(fields.shape[0]), int(fields.shape[1]), int(fields.shape[2])
+    overlap = int(overlap)
+    if overlap < 0 or 2 * overlap > t:
+        raise ApicError("overlap must satisfy 0 <= 2 overlap <= T")
+    lib = load()
+    h, w = ty * (t - overlap) + overlap, tx * (t - overlap) + overlap
+    fov = out if out is not None else torch.empty((h, w), dtype=torch.complex64, device=fields.device)
+    if not (fov.is_cuda and fov.dtype == torch.complex64 and fov.is_contiguous() and tuple(fov.shape) == (h, w)):
+        raise ApicError("out must be a contiguous complex64 CUDA tensor [H][W]")
+    factors = torch.empty((ty, tx), dtype=torch.complex64, device=fields.device)
+    work = torch.empty((max(1, lib.apic_reassemble_work_bytes(ty, tx)),), dtype=torch.uint8, device=fields.device)
+    stream = torch.cuda.current_stream(fields.device).cuda_stream
+    _check(lib.apic_reassemble(fields.data_ptr(), ty, tx, t, overlap, int(bool(align)), fov.data_ptr(), factors.data_ptr(),
+                               work.data_ptr(), C.c_void_p(stream)), "apic_reassemble")
+    return fov, factors
 
 
 def fft2d(x, inverse: bool = False):
