@@ -406,9 +406,14 @@ def weighted_solve(a: np.ndarray, b: np.ndarray, w: np.ndarray) -> np.ndarray:
     return np.linalg.solve(a.T @ aw, aw.T @ b)
 
 
-def solve_aberration(geo: Geometry, spectra_centred: Sequence[np.ndarray], refine_iters: int):
+def solve_aberration(geo: Geometry, spectra_centred: Sequence[np.ndarray], refine_iters: int,
+                     c_init: Optional[np.ndarray] = None):
     """O4.  spectra_centred[i] = S_hat_i on the centred grid (only D_i is read).
-    Returns (c [n_z], status, info dict with row counts / residual)."""
+    Returns (c [n_z], status, info dict with row counts / residual).
+    c_init (reading B9: "initialise S6 from neighbours"; the paper shows the pupil
+    varying smoothly over the slide, Fig. 4(b)): a prior for the coefficients, e.g. the slide-level fit
+    of pupil_field_fit evaluated at this tile.  It REPLACES the gradient-domain start c^0; the re-wrapped refinement
+    steps and the status rule are unchanged, so inside the basin of R11 the result is the same minimiser."""
     full_a, full_beta, full_w = [], [], []
     grad_a, grad_b, grad_w = [], [], []
     for (i, l) in geo.pairs:
@@ -433,7 +438,10 @@ def solve_aberration(geo: Geometry, spectra_centred: Sequence[np.ndarray], refin
     beta = np.concatenate(full_beta)
     w_full = np.concatenate(full_w)
     a_grad = np.concatenate(grad_a)
-    c = weighted_solve(a_grad, np.concatenate(grad_b), np.concatenate(grad_w))     # c^0
+    if c_init is None:
+        c = weighted_solve(a_grad, np.concatenate(grad_b), np.concatenate(grad_w))  # c^0
+    else:
+        c = np.asarray(c_init, dtype=np.float64).copy()                              # B9
     normal = a_full.T @ (a_full * w_full[:, None])
     for _ in range(refine_iters):                                                  # (ii)
         r = wrap_phase(beta - a_full @ c)
@@ -588,7 +596,8 @@ class OracleResult:
 
 
 def reconstruct_tile(stack: np.ndarray, p: OracleParams, geo: Optional[Geometry] = None,
-                     sets: Optional[List[DarkSets]] = None, keep: bool = False) -> OracleResult:
+                     sets: Optional[List[DarkSets]] = None, keep: bool = False,
+                     zernike_init: Optional[np.ndarray] = None) -> OracleResult:
     """The whole hot path O1..O7 for one tile.  stack: [n_bright+n_dark][N][N]."""
     n = p.tile_n
     nb = len(p.k_bright)
@@ -607,7 +616,7 @@ def reconstruct_tile(stack: np.ndarray, p: OracleParams, geo: Optional[Geometry]
     for i in range(nb):                                                       # O2, O3
         s = kk_field(x[i], geo.kappa_b[i], floor=p.intensity_floor, pad=p.kk_pad)
         spectra.append(np.where(geo.disc_b[i], np.fft.fftshift(sub_spectrum(s)), 0.0))
-    coef, status, info = solve_aberration(geo, spectra, p.refine_iters)      # O4
+    coef, status, info = solve_aberration(geo, spectra, p.refine_iters, c_init=zernike_init)   # O4 (B9)
     o_hat, known = stitch(geo, spectra, coef)                                 # O5
     if len(p.k_dark):
         o_hat, known = darkfield_extend(geo, o_hat, known, coef, x[nb:], sets=sets)   # O6
