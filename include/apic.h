@@ -221,6 +221,22 @@ int apic_submit_host_u16(apic_plan* plan, int slot, const uint16_t* h_raw, const
                          float* h_field, float* h_zernike, float* h_pupil, int32_t* h_status);
 int apic_wait_host(apic_plan* plan, int slot);
 
+/* Slide-level pupil prior (PAPER.md:171 / Fig. 4(b): the recovered pupil varies smoothly over
+ * the slide; the use made of it is reading B9 of DESIGN.md).
+ * apic_pupil_field_fit: d_zernike [tiles][n_zernike] (what apic_reconstruct returned), d_status [tiles], d_xy [tiles][2]
+ * (slide coordinates of the tiles, any units; [-1, 1] keeps the fit well scaled) -> d_fit [tiles][n_zernike]: each
+ * coefficient's least-squares polynomial of total degree `order` (0, 1, 2; terms 1, X, Y, X^2, XY, Y^2) over the tiles
+ * with status 0, evaluated at EVERY tile; d_poly [6][n_zernike] the polynomial (unused terms 0).  If those tiles do not
+ * determine the polynomial: their mean; none: zeros.  One small kernel on cuda_stream; device pointers; n_zernike <= 64.
+ * apic_reconstruct_prior: apic_reconstruct whose aberration fit (S6) starts from d_zernike_init [batch][n_zernike]
+ * (e.g. the rows of d_fit) instead of its own gradient-domain start; the re-wrapped refinement steps and the status
+ * rule are unchanged, so a tile inside the basin of its own start gets the same coefficients, and a tile whose own
+ * start lands in a wrong minimum (large aberrations on small tiles, R11) is rescued by its neighbours. */
+int apic_pupil_field_fit(const float* d_zernike, const int32_t* d_status, const float* d_xy, int tiles, int n_zernike,
+                         int order, float* d_fit, float* d_poly, void* cuda_stream);
+int apic_reconstruct_prior(apic_plan* plan, const float* d_intensity, const float* d_zernike_init, int batch,
+                           float* d_field, float* d_zernike, float* d_pupil, int32_t* d_status, void* cuda_stream);
+
 /* Within-FOV reassembly of overlapping reconstructed tiles ("individually
  * reconstructed and then stitched together", "the overlapping regions were blended"; the blend and the
  * global-phase treatment are readings B6-B8 of DESIGN.md).  d_fields: [tiles_y][tiles_x][tile_px][tile_px] complex64

@@ -26,7 +26,7 @@ EXPORTS = ("apic_params_default", "apic_plan_create", "apic_plan_destroy", "apic
            "apic_debug_buffer", "apic_debug_copy", "apic_fft2d", "apic_fft2d_xy", "apic_last_launch_count", "apic_strerror",
            "apic_last_cuda_error", "apic_version", "apic_profile_categories", "apic_profile_category_name",
            "apic_profile_begin", "apic_profile_end", "apic_profile_work", "apic_measure_peak", "apic_reassemble",
-           "apic_reassemble_work_bytes")
+           "apic_reassemble_work_bytes", "apic_pupil_field_fit", "apic_reconstruct_prior")
 
 
 class ApicError(RuntimeError):
@@ -101,6 +101,10 @@ def load() -> C.CDLL:
                                      C.POINTER(C.c_longlong)]
     lib.apic_profile_work.argtypes = [C.c_void_p, C.POINTER(C.c_ulonglong)]
     lib.apic_measure_peak.argtypes = [C.c_int, C.POINTER(C.c_double), C.c_void_p]
+    lib.apic_pupil_field_fit.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
+                                         C.c_void_p]
+    lib.apic_reconstruct_prior.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
+                                           C.c_void_p, C.c_void_p]
     lib.apic_reassemble_work_bytes.argtypes = [C.c_int, C.c_int]
     lib.apic_reassemble_work_bytes.restype = C.c_size_t
     lib.apic_reassemble.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
@@ -195,9 +199,11 @@ class Plan:
         _check(self._lib.apic_plan_dark_sets(self._h, led, nu, nq), "apic_plan_dark_sets")
         return [(led[i], nu[i], nq[i]) for i in range(n)]
 
-    def reconstruct(self, intensity, want_pupil: bool = True, out=None):
+    def reconstruct(self, intensity, want_pupil: bool = True, out=None, zernike_init=None):
         """intensity: float32 CUDA tensor [B][n_img][N][N].  Returns (field complex64 [B][uN][uN],
-        zernike float32 [B][nz], pupil complex64 [B][N][N] | None, status int32 [B])."""
+        zernike float32 [B][nz], pupil complex64 [B][N][N] | None, status int32 [B]).
+        zernike_init: float32 CUDA tensor [B][nz], a prior that replaces the start of the aberration fit
+        (apic_reconstruct_prior)."""
         import torch
         if not (intensity.is_cuda and intensity.dtype == torch.float32 and intensity.is_contiguous()):
             raise ApicError("intensity must be a contiguous float32 CUDA tensor")
@@ -213,6 +219,14 @@ class Plan:
         else:
             field, zern, pupil, status = out
         stream = torch.cuda.current_stream(dev).cuda_stream
+        if zernike_init is not None:
+            if not (zernike_init.is_cuda and zernike_init.dtype == torch.float32 and zernike_init.is_contiguous()
+                    and tuple(zernike_init.shape) == (b, self.nz)):
+                raise ApicError(f"zernike_init must be a contiguous float32 CUDA tensor [{b},{self.nz}]")
+            _check(self._lib.apic_reconstruct_prior(self._h, intensity.data_ptr(), zernike_init.data_ptr(), b, field.data_ptr(),
+                                                    zern.data_ptr(), pupil.data_ptr() if pupil is not None else None,
+                                                    status.data_ptr(), C.c_void_p(stream)), "apic_reconstruct_prior")
+            return field, zern, pupil, status
         _check(self._lib.apic_reconstruct(self._h, intensity.data_ptr(), b, field.data_ptr(), zern.data_ptr(),
                                           pupil.data_ptr() if pupil is not None else None, status.data_ptr(),
                                           C.c_void_p(stream)), "apic_reconstruct")
@@ -345,6 +359,23 @@ def measure_peak(what: int) -> float:
     _check(load().apic_measure_peak(int(what), C.byref(v), C.c_void_p(torch.cuda.current_stream().cuda_stream)),
            "apic_measure_peak")
     return float(v.value)
+
+
+def pupil_field_fit(zernike, status, xy, order: int = 2):
+    """apic_pupil_field_fit: zernike float32 CUDA [T][nz], status int32 CUDA [T], xy float32 CUDA [T][2].
+    Returns (fit float32 [T][nz], poly float32 [6][nz])."""
+    import torch
+    t, nz = int(zernike.shape[0]), int(zernike.shape[1])
+    if not (zernike.is_cuda and zernike.dtype == torch.float32 and zernike.is_contiguous()
+            and status.is_cuda and status.dtype == torch.int32 and status.is_contiguous() and tuple(status.shape) == (t,)
+            and xy.is_cuda and xy.dtype == torch.float32 and xy.is_contiguous() and tuple(xy.shape) == (t, 2)):
+        raise ApicError("zernike float32 [T][nz], status int32 [T], xy float32 [T][2]: contiguous CUDA tensors")
+    fit = torch.empty_like(zernike)
+    poly = torch.empty((6, nz), dtype=torch.float32, device=zernike.device)
+    stream = torch.cuda.current_stream(zernike.device).cuda_stream
+    _check(load().apic_pupil_field_fit(zernike.data_ptr(), status.data_ptr(), xy.data_ptr(), t, nz, int(order), fit.data_ptr(),
+                                       poly.data_ptr(), C.c_void_p(stream)), "apic_pupil_field_fit")
+    return fit, poly
 
 
 def reassemble(fields, overlap: int, align: bool = True, out=None):

@@ -15,7 +15,7 @@ PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 OBJ = PKG / "build"
 LIB = PKG / "libapic.so"
-SOURCES = ["geometry.cpp", "api.cu", "kk.cu", "aberration.cu", "df_team.cu", "df_mgrid.cu", "df_tma.cu", "df_wide.cu", "output.cu", "peaks.cu", "reassemble.cu"]
+SOURCES = ["geometry.cpp", "api.cu", "kk.cu", "aberration.cu", "df_team.cu", "df_mgrid.cu", "df_tma.cu", "df_wide.cu", "output.cu", "peaks.cu", "reassemble.cu", "pupil_prior.cu"]
 HEADERS = ["geometry.hpp", "plan.hpp", "fft_core.cuh", "fft_xy.cuh", "../../include/apic.h"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
               "-Xcompiler", "-fPIC"] + os.environ.get("APIC_EXTRA_NVCC_FLAGS", "").split()

@@ -197,8 +197,18 @@ __global__ void __launch_bounds__(128) ab_solve(DevTables t, const float* __rest
   }
 }
 
+// B9: the fit starts from a prior (one per tile) instead of the gradient-domain solve
+__global__ void ab_set_init(int nz, const float* __restrict__ init, float* __restrict__ coef, int32_t* __restrict__ fail,
+                            const int32_t* __restrict__ live, const int32_t* __restrict__ live_count, int chunk0) {
+  const int slot = blockIdx.x;
+  const int tile = resolve_tile_idx(live, live_count, chunk0, slot);
+  if (tile < 0) return;
+  if (threadIdx.x < nz) coef[size_t(slot) * nz + threadIdx.x] = init[size_t(tile) * nz + threadIdx.x];
+  if (threadIdx.x == 0) fail[slot] = 0;
+}
+
 void launch_aberration(const DevTables& t, const Workspace& w, const LaunchCtx& c, int refine_iters,
-                       float* d_zernike, int32_t* d_status) {
+                       float* d_zernike, int32_t* d_status, const float* d_init) {
   const size_t sm = (size_t(kGramRows) * ((t.nz + 2) | 1) + size_t(w.gram_entries)) * sizeof(float);
   if (!c.pd->attr_ab) {
     cudaFuncSetAttribute(ab_gram<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
@@ -209,12 +219,17 @@ void launch_aberration(const DevTables& t, const Workspace& w, const LaunchCtx& 
   { ProfScope ps(c, CAT_AB_PRODUCTS);
     ab_pair_products<<<g1, 256, 0, c.stream>>>(t, w.S, w.PR, c.live_count, c.chunk0); }
   const int parts_g = (t.n_grad + kGramRows - 1) / kGramRows, parts_f = (t.n_rows + kGramRows - 1) / kGramRows;
-  { ProfScope ps(c, CAT_AB_GRAM);
-    ab_gram<0><<<dim3(parts_g, c.chunk_tiles), 256, sm, c.stream>>>(t, w.PR, w.coef, w.gram, parts_g, w.gram_entries,
-                                                                      c.live_count, c.chunk0); }
-  { ProfScope ps(c, CAT_AB_SOLVE);
-    ab_solve<0><<<c.chunk_tiles, 128, 0, c.stream>>>(t, w.gram, parts_g, w.gram_entries, w.coef, w.ab_fail, d_zernike,
-                                                     d_status, c.live, c.live_count, c.chunk0); }
+  if (d_init) {
+    ProfScope ps(c, CAT_AB_SOLVE);
+    ab_set_init<<<c.chunk_tiles, 64, 0, c.stream>>>(t.nz, d_init, w.coef, w.ab_fail, c.live, c.live_count, c.chunk0);
+  } else {
+    { ProfScope ps(c, CAT_AB_GRAM);
+      ab_gram<0><<<dim3(parts_g, c.chunk_tiles), 256, sm, c.stream>>>(t, w.PR, w.coef, w.gram, parts_g, w.gram_entries,
+                                                                        c.live_count, c.chunk0); }
+    { ProfScope ps(c, CAT_AB_SOLVE);
+      ab_solve<0><<<c.chunk_tiles, 128, 0, c.stream>>>(t, w.gram, parts_g, w.gram_entries, w.coef, w.ab_fail, d_zernike,
+                                                       d_status, c.live, c.live_count, c.chunk0); }
+  }
   for (int it = 0; it <= refine_iters; ++it) {
     { ProfScope ps(c, CAT_AB_GRAM);
       ab_gram<1><<<dim3(parts_f, c.chunk_tiles), 256, sm, c.stream>>>(t, w.PR, w.coef, w.gram, parts_f,

@@ -417,7 +417,7 @@ int apic_plan_dark_sets(const apic_plan* plan, int* led, int* n_unknown, int* n_
 // The whole path on workspace set `zi`.  `src` holds either fp32 intensities or uint16 counts + per-image scale;
 // the uint16 form is converted in the loads of S0, S1 and S8 (no fp32 working copy).
 static int reconstruct_impl(apic_plan* plan, int zi, const ImgSrc& src, int batch, float* d_field, float* d_zernike,
-                            float* d_pupil, int32_t* d_status, cudaStream_t s) {
+                            float* d_pupil, int32_t* d_status, cudaStream_t s, const float* d_init = nullptr) {
   if (!plan || !(src.f32 || (src.u16 && src.scale)) || !d_field || !d_zernike || !d_status) return APIC_EINVAL;
   if (batch < 1 || batch > plan->params.max_batch) return APIC_EBATCH;
   WsSet& z = plan->set[zi];
@@ -455,7 +455,7 @@ static int reconstruct_impl(apic_plan* plan, int zi, const ImgSrc& src, int batc
     LaunchCtx c{s, &plan->launches, &plan->prof, z.bs.live, z.bs.live_count, c0, std::min(per_pass, n_live - c0),
                 &plan->pd, z.aux, z.ev_fork, z.ev_join};
     launch_kk(t, w, c, src, z.bs.stats, p.intensity_floor);                                   // S1-S5
-    launch_aberration(t, w, c, p.refine_iters, d_zernike, d_status);                          // S6
+    launch_aberration(t, w, c, p.refine_iters, d_zernike, d_status, d_init);                  // S6
     launch_stitch(t, w, c);                                                                   // S7
     if ((p.df_mode == 0 || p.df_mode == 5) && t.n == 256) {                                   // S8-S10
       // df_wide.cu: mode 0 = 256-thread CTAs at 128 registers (groups 11), mode 5 = 1024-thread CTA pairs (groups 4)
@@ -480,6 +480,14 @@ int apic_reconstruct(apic_plan* plan, const float* d_intensity, int batch, float
   DeviceGuard guard(plan->pd.device);
   return reconstruct_impl(plan, 0, ImgSrc{d_intensity, nullptr, nullptr}, batch, d_field, d_zernike, d_pupil, d_status,
                           static_cast<cudaStream_t>(cuda_stream));
+}
+
+int apic_reconstruct_prior(apic_plan* plan, const float* d_intensity, const float* d_zernike_init, int batch, float* d_field,
+                           float* d_zernike, float* d_pupil, int32_t* d_status, void* cuda_stream) {
+  if (!plan || !d_intensity || !d_zernike_init) return APIC_EINVAL;
+  DeviceGuard guard(plan->pd.device);
+  return reconstruct_impl(plan, 0, ImgSrc{d_intensity, nullptr, nullptr}, batch, d_field, d_zernike, d_pupil, d_status,
+                          static_cast<cudaStream_t>(cuda_stream), d_zernike_init);
 }
 
 int apic_reconstruct_u16(apic_plan* plan, const uint16_t* d_raw, const float* d_scale, int batch, float* d_field,

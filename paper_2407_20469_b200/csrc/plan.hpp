@@ -177,8 +177,9 @@ void launch_zero_dead(const DevTables& t, const int32_t* status, int batch, floa
 void launch_kk(const DevTables& t, const Workspace& w, const LaunchCtx& c, const ImgSrc& src,
                const double* stats, float floor_rel);
 // aberration (S6) + stitching (S7)
+// d_init != nullptr: [batch][nz] prior coefficients (indexed by tile) that replace the gradient-domain start (reading B9)
 void launch_aberration(const DevTables& t, const Workspace& w, const LaunchCtx& c, int refine_iters,
-                       float* d_zernike, int32_t* d_status);
+                       float* d_zernike, int32_t* d_status, const float* d_init = nullptr);
 void launch_stitch(const DevTables& t, const Workspace& w, const LaunchCtx& c);
 // darkfield (S8-S10), every LED in one launch (df_team.cu)
 void launch_darkfield_team(const DevTables& t, const DarkDev* d_leds, int n_leds, const Workspace& w, const LaunchCtx& c,
