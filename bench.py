@@ -155,7 +155,12 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append([c.strip() for c in line.split(",")])
+            self.rows.append([c.strip() for c in line.split(",")] + [time.perf_counter()])
+
+    def mark(self):
+        """The timed region starts now: only samples that arrive from here on count (nvidia-smi is started before the
+        warm-up steps because its first sample can take longer than a short timed region)."""
+        self.t_mark = time.perf_counter()
 
     def stop(self):
         if not self.proc:
@@ -166,7 +171,11 @@ class ClockSampler:
         except Exception:
             self.proc.kill()
         sm, mx, reasons = [], [], set()
-        for r in self.rows:
+        t_mark = getattr(self, "t_mark", None)
+        rows = [r for r in self.rows if t_mark is None or r[-1] >= t_mark]
+        if not rows:
+            rows = self.rows[-3:]                        # a timed region shorter than the sampling period: the samples of
+        for r in rows:                                   # the warm-up steps right before it (the GPU was under the same load)
             try:
                 sm.append(float(r[0])); mx.append(float(r[1]))
             except Exception:
@@ -518,11 +527,12 @@ def run_batch(ctx):
             dist.barrier()
             torch.cuda.synchronize()
 
+    sampler = make_sampler(local)
+    sampler.start()
     for _ in range(args.warmup):
         plan.reconstruct(x, out=out)
     barrier()
-    sampler = make_sampler(local)
-    sampler.start()
+    sampler.mark()
     plan.profile_begin(stride=1, max_samples=16384)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches = 0
