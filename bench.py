@@ -553,7 +553,7 @@ def run_batch(ctx):
                          "the throughput of a failed step is not a result")
     mpx = world * args.steps * tiles * on * on / 1e6 / (ms / 1e3)
     chunk = plan.info["chunk_tiles"]
-    workload = f"cfg{args.config}_{tiles}tiles"
+    workload = f"cfg{args.config}_{tiles}tiles" + (f"_mode{args.df_mode}" if args.df_mode else "")   # tag of the ncu rows under profiles/
     algo_bytes = tiles * (host[0].nbytes + on * on * 8 + n * n * 8 + nz * 4 + 4)
     roofline = roofline_line(ctx, plan, prof, clocks, tiles, workload, ms / args.steps, algo_bytes)
 
