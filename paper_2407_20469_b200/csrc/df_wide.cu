@@ -72,6 +72,7 @@ struct Args {
   unsigned long long* tl;     // optional timeline of team 0 (APIC_DF_TIMELINE=<file>): [cta][group][kTlCap] clock marks
 };
 constexpr int kTlCap = 8192;
+#ifdef APIC_TIMELINE   // debugging aid: build with APIC_EXTRA_NVCC_FLAGS=-DAPIC_TIMELINE, run with APIC_DF_TIMELINE=<file>
 #define WD_MARK(id)                                                                                   \
   do {                                                                                                \
     if (a.tl && team_id == 0 && g.tid == 0 && tl_n + 1 < kTlCap) {                                    \
@@ -80,6 +81,9 @@ constexpr int kTlCap = 8192;
       a.tl[(size_t(cr) * NG + g.grp) * kTlCap + ++tl_n] = (t_ << 8) | unsigned(id);                   \
     }                                                                                                 \
   } while (0)
+#else
+#define WD_MARK(id) do {} while (0)
+#endif
 
 __device__ __forceinline__ unsigned cluster_rank() {
   unsigned r;
@@ -923,6 +927,7 @@ __device__ __forceinline__ float2 vr_block_sum2(float a, float b, float2* red, i
 template <int NG>
 __device__ __noinline__ int vr_cg(const Args& a, const Ctx c, unsigned cr, float2* tm_t, const float2* pf_t, const float2* s0g,
                                   double& flop, bool mark, int& tl_n) {
+#ifdef APIC_TIMELINE
 #define VR_MARK(id)                                                                                   \
   do {                                                                                                \
     if (mark && threadIdx.x == 0 && tl_n + 1 < kTlCap) {                                              \
@@ -931,6 +936,9 @@ __device__ __noinline__ int vr_cg(const Args& a, const Ctx c, unsigned cr, float
       a.tl[(size_t(cr) * NG) * kTlCap + ++tl_n] = (t_ << 8) | unsigned(id);                           \
     }                                                                                                 \
   } while (0)
+#else
+#define VR_MARK(id) do {} while (0)
+#endif
   constexpr int NT = NG * GT;
   const DarkDev& L = *c.Lp();
   const Vr g = vr_geometry(L, c, NG);
@@ -1088,7 +1096,6 @@ __global__ void __launch_bounds__(NG * GT, MINB) df_wide_kernel(const __grid_con
       const int n_d = (Lsh.d_nrow + 15) >> 4, n_q = (Lsh.q_nrow + 15) >> 4, n_u = (Lsh.u_nrow + 15) >> 4, n_c = Lsh.mx >> 4;
       if (g.sigma < n_q) { WD_R1_SWITCH(r1x, c.kq(g.grp)[g.tid] = q_keep_bits<R>(Lsh, g.sigma, g.tid)); }
       __syncthreads();
-      const double fx = 16.0 * line_flop(Lsh.mx), fy = 16.0 * line_flop(Lsh.my), fn = 16.0 * line_flop(N);
       // ---- setup: P_hat -> p_N, p_M -> d on Q -> s = C^H d
       WD_MARK(100 + k);
       ph_build_p_rows_n(c, g, o_t, tn_t, nz);
@@ -1114,10 +1121,13 @@ __global__ void __launch_bounds__(NG * GT, MINB) df_wide_kernel(const __grid_con
       WD_MARK(28);
       team_sync(multi);
       WD_MARK(29);
-      flop += mine(n_d) * (fn + fx) + mine(N / 16) * 2 * fn + mine(n_c) * fy + mine(n_q) * (fn + fx) + mine(n_c) * 2 * fy +
-              mine(n_u) * fx;
+      if (g.tid == 0) {
+        const double fx = 16.0 * line_flop(Lsh.mx), fy = 16.0 * line_flop(Lsh.my), fn = 16.0 * line_flop(N);
+        flop += mine(n_d) * (fn + fx) + mine(N / 16) * 2 * fn + mine(n_c) * fy + mine(n_q) * (fn + fx) + mine(n_c) * 2 * fy +
+                mine(n_u) * fx;
+      }
       int iters = 0;
-      const bool use_vr = a.vr && G == 2 && vr_fits(Lsh, c, NG, a.vr_mu);
+      const bool use_vr = NG == 4 && a.vr && G == 2 && vr_fits(Lsh, c, NG, a.vr_mu);   // compiled into the 1024-thread shape only
       if (use_vr) {
         // s0 = C^H d sits in VW (global; the wide set-up wrote it before the barrier above): both CTAs take all of it
         iters = vr_cg<NG>(a, c, cr, tm_t, pf_t, V.w.p, flop, a.tl && team_id == 0, tl_n);
@@ -1161,7 +1171,6 @@ __global__ void __launch_bounds__(NG * GT, MINB) df_wide_kernel(const __grid_con
         WD_MARK(10);
         team_sync(multi);
         WD_MARK(11);
-        flop += 2 * mine(n_u) * fx + 4 * mine(n_c) * fy + 2 * mine(n_q) * fx;
         ++iters;
         const float4 tot = cg_totals(c, n_u);              // <pdir, w>, <s, w>, <w, w>, <s, s>
         if (!(tot.x > 0.f)) break;
@@ -1171,6 +1180,9 @@ __global__ void __launch_bounds__(NG * GT, MINB) df_wide_kernel(const __grid_con
         WD_MARK(12);
         done = !(gnew > a.tol2 * gamma0);
       }
+      if (g.tid == 0)                                      // executed line transforms of the loop (nothing of this is live inside it)
+        flop += double(iters) * (2 * mine(n_u) * 16.0 * line_flop(Lsh.mx) + 4 * mine(n_c) * 16.0 * line_flop(Lsh.my) +
+                                 2 * mine(n_q) * 16.0 * line_flop(Lsh.mx));
       gsync(g);
       // ---- S10: O_hat(u) = U_hat(u) e^{-j phi(u+kappa)}, known ∪= U (every slot extends with its share)
       {
