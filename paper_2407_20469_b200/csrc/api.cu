@@ -236,7 +236,10 @@ int apic_plan_destroy(apic_plan* plan) {
   DeviceGuard guard(plan->pd.device);
   for (void* q : plan->allocs) cudaFree(q);
   for (cudaEvent_t e : plan->prof.ev) cudaEventDestroy(e);
-  for (WsSet& z : plan->set) if (z.h_live_count) cudaFreeHost(z.h_live_count);
+  for (WsSet& z : plan->set) {
+    if (z.h_live_count) cudaFreeHost(z.h_live_count);
+    if (z.aux) { cudaStreamDestroy(z.aux); cudaEventDestroy(z.ev_fork); cudaEventDestroy(z.ev_join); }
+  }
   cudaFree(plan->st_int); cudaFree(plan->st_field); cudaFree(plan->st_zern); cudaFree(plan->st_pupil);
   cudaFree(plan->st_status);
   cudaFree(plan->st_raw); cudaFree(plan->st_scale);
