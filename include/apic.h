@@ -43,7 +43,8 @@ typedef enum {
   APIC_EINVAL = -1,   /* bad parameter / geometry (see apic_plan_create) */
   APIC_ECUDA = -2,    /* a CUDA runtime call failed (apic_last_cuda_error gives the text) */
   APIC_ENOMEM = -3,   /* host or device allocation failed */
-  APIC_EBATCH = -4    /* batch outside 1..max_batch */
+  APIC_EBATCH = -4,   /* batch outside 1..max_batch */
+  APIC_ESCRATCH = -5  /* problem larger than the scratch built into the library (apic_reassemble_static) */
 } apic_error;
 
 /* Per-tile status written to d_status. */
@@ -251,6 +252,32 @@ int apic_reconstruct_prior(apic_plan* plan, const float* d_intensity, const floa
 size_t apic_reassemble_work_bytes(int tiles_y, int tiles_x);
 int apic_reassemble(const float* d_fields, int tiles_y, int tiles_x, int tile_px, int overlap, int align, float* d_fov,
                     float* d_factors, void* d_work, void* cuda_stream);
+
+/* apic_reassemble for callers that cannot supply d_work because they cannot obtain device memory at the point
+ * where they reassemble: a host program that gave all device memory to its own arena at start-up, a component
+ * whose embedding application owns the allocator, a real-time acquisition loop in which a cudaMalloc / cudaFree
+ * would stall every stream of the process.  Same arguments, same kernels and bit-identical results to
+ * apic_reassemble, minus d_work: the scratch is a fixed array compiled into libapic's device image.
+ *  - Limit: tiles_y * tiles_x <= apic_reassemble_static_max_tiles() (1024, e.g. a 32 x 32 FOV); beyond it the
+ *    call returns APIC_ESCRATCH and enqueues nothing - use apic_reassemble with your own d_work then.  Every
+ *    other argument is validated as in apic_reassemble (APIC_EINVAL).
+ *  - Cost: the array (528 KiB) occupies memory on every GPU on which this library's device code gets loaded,
+ *    from that moment until the process ends, used or not.
+ *  - The call itself performs no cudaMalloc / cudaFree and calls no library routine that allocates; d_fields,
+ *    d_fov and d_factors remain the caller's DEVICE buffers.
+ *  - Set-up: the FIRST call on each device asks the CUDA runtime for the array's address on that device
+ *    (cudaGetSymbolAddress, host-synchronous, may load the library's device code) and caches it; later calls
+ *    on that device only enqueue the three kernels.  The device that owns the buffers must be current during
+ *    every call.  Make that first call during initialisation, outside any stream capture.  A failed look-up
+ *    returns APIC_ECUDA (text in apic_last_cuda_error) and is retried by the next call.
+ *  - Sharing: all calls on one device, from any thread, stream or plan-less context, use the SAME array.  Calls
+ *    whose kernels can overlap on the GPU (different streams without an ordering event between them) race on it
+ *    and both results are undefined; order them on one stream or with events.  The array keeps whatever the last
+ *    call wrote; no call depends on it (every element read is written earlier in the same call), so nothing is
+ *    cleared between calls. */
+int apic_reassemble_static_max_tiles(void);
+int apic_reassemble_static(const float* d_fields, int tiles_y, int tiles_x, int tile_px, int overlap, int align,
+                           float* d_fov, float* d_factors, void* cuda_stream);
 
 /* Stage-level access for parity tests (device pointers, valid after apic_reconstruct on the
  * same stream, for the tiles of the LAST internal chunk; tile index is chunk-local):

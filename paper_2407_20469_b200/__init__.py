@@ -16,7 +16,7 @@ import numpy as np
 _PKG = Path(__file__).resolve().parent
 LIB_PATH = _PKG / "libapic.so"
 
-APIC_OK, APIC_EINVAL, APIC_ECUDA, APIC_ENOMEM, APIC_EBATCH = 0, -1, -2, -3, -4
+APIC_OK, APIC_EINVAL, APIC_ECUDA, APIC_ENOMEM, APIC_EBATCH, APIC_ESCRATCH = 0, -1, -2, -3, -4, -5
 TILE_OK, TILE_BACKGROUND, TILE_BAD_INPUT, TILE_SOLVE_FAILED = 0, 1, 2, 3
 DBG_SUBSPECTRA, DBG_OBJECT_SPECTRUM, DBG_DF_ITERS = 0, 1, 2
 
@@ -26,7 +26,8 @@ EXPORTS = ("apic_params_default", "apic_plan_create", "apic_plan_destroy", "apic
            "apic_debug_buffer", "apic_debug_copy", "apic_fft2d", "apic_fft2d_xy", "apic_last_launch_count", "apic_strerror",
            "apic_last_cuda_error", "apic_version", "apic_profile_categories", "apic_profile_category_name",
            "apic_profile_begin", "apic_profile_end", "apic_profile_work", "apic_measure_peak", "apic_reassemble",
-           "apic_reassemble_work_bytes", "apic_pupil_field_fit", "apic_reconstruct_prior")
+           "apic_reassemble_work_bytes", "apic_reassemble_static", "apic_reassemble_static_max_tiles",
+           "apic_pupil_field_fit", "apic_reconstruct_prior")
 
 
 class ApicError(RuntimeError):
@@ -109,6 +110,9 @@ def load() -> C.CDLL:
     lib.apic_reassemble_work_bytes.restype = C.c_size_t
     lib.apic_reassemble.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p,
                                     C.c_void_p]
+    lib.apic_reassemble_static_max_tiles.argtypes = []
+    lib.apic_reassemble_static.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p,
+                                           C.c_void_p]
     _lib = lib
     return lib
 
@@ -400,6 +404,45 @@ def reassemble(fields, overlap: int, align: bool = True, out=None):
     _check(lib.apic_reassemble(fields.data_ptr(), ty, tx, t, overlap, int(bool(align)), fov.data_ptr(), factors.data_ptr(),
                                work.data_ptr(), C.c_void_p(stream)), "apic_reassemble")
     return fov, factors
+
+
+def reassemble_static(fields, overlap: int, align: bool = True, out=None, factors=None):
+    """apic_reassemble_static: ``reassemble`` for callers that must not allocate device memory where they reassemble
+    (a process whose GPU memory is already handed out in full, or a loop that cannot afford the stall of an
+    allocation).  The library keeps the scratch in a fixed array inside its own device image, so the FOV is limited
+    to ``reassemble_static_max_tiles()`` tiles (ApicError with APIC_ESCRATCH beyond that), all calls on a device share
+    that array (do not let two of them overlap on the GPU), and the first call on a device does a one-off, host-side
+    address look-up: make it at start-up.  Pass preallocated ``out`` [H][W] and ``factors`` [tiles_y][tiles_x]
+    (complex64, CUDA, contiguous) and this wrapper allocates nothing either; left out, they are created with torch
+    for convenience.  Returns (fov, factors), bit-identical to ``reassemble``."""
+    import torch
+    if not (fields.is_cuda and fields.dtype == torch.complex64 and fields.is_contiguous() and fields.dim() == 4
+            and fields.shape[2] == fields.shape[3]):
+        raise ApicError("fields must be a contiguous complex64 CUDA tensor [tiles_y][tiles_x][T][T]")
+    ty, tx, t = int(fields.shape[0]), int(fields.shape[1]), int(fields.shape[2])
+    overlap = int(overlap)
+    if overlap < 0 or 2 * overlap > t:
+        raise ApicError("overlap must satisfy 0 <= 2 overlap <= T")
+    h, w = ty * (t - overlap) + overlap, tx * (t - overlap) + overlap
+    fov = out if out is not None else torch.empty((h, w), dtype=torch.complex64, device=fields.device)
+    if not (fov.is_cuda and fov.dtype == torch.complex64 and fov.is_contiguous() and tuple(fov.shape) == (h, w)
+            and fov.device == fields.device):
+        raise ApicError("out must be a contiguous complex64 CUDA tensor [H][W] on the device of fields")
+    u = factors if factors is not None else torch.empty((ty, tx), dtype=torch.complex64, device=fields.device)
+    if not (u.is_cuda and u.dtype == torch.complex64 and u.is_contiguous() and tuple(u.shape) == (ty, tx)
+            and u.device == fields.device):
+        raise ApicError("factors must be a contiguous complex64 CUDA tensor [tiles_y][tiles_x] on the device of fields")
+    lib = load()
+    with torch.cuda.device(fields.device):      # the address look-up and the launches need the buffers' device current
+        stream = torch.cuda.current_stream(fields.device).cuda_stream
+        _check(lib.apic_reassemble_static(fields.data_ptr(), ty, tx, t, overlap, int(bool(align)), fov.data_ptr(),
+                                          u.data_ptr(), C.c_void_p(stream)), "apic_reassemble_static")
+    return fov, u
+
+
+def reassemble_static_max_tiles() -> int:
+    """Largest tiles_y * tiles_x that ``reassemble_static`` accepts (the size of the built-in scratch)."""
+    return int(load().apic_reassemble_static_max_tiles())
 
 
 def fft2d(x, inverse: bool = False):

@@ -28,6 +28,11 @@ bool cuda_ok(cudaError_t e, const char* what) {
 
 }  // namespace
 
+namespace apic {
+// for the translation units that have no plan (reassemble.cu): same text slot as cuda_ok()
+void note_cuda_error(cudaError_t e, const char* what) { cuda_ok(e == cudaSuccess ? cudaErrorUnknown : e, what); }
+}  // namespace apic
+
 // One workspace set: everything a pass of apic_reconstruct writes.  The plan owns two; the second is
 // allocated on first use by apic_reconstruct_host so that the kernels of one sub-batch run beside the
 // copies (and the kernels) of its neighbours.
@@ -197,6 +202,9 @@ const char* apic_strerror(int err) {
     case APIC_ECUDA: return "CUDA runtime error (see apic_last_cuda_error)";
     case APIC_ENOMEM: return "out of memory";
     case APIC_EBATCH: return "batch outside 1..max_batch";
+    case APIC_ESCRATCH:
+      return "more tiles than the library's built-in scratch holds (apic_reassemble_static_max_tiles); use apic_reassemble "
+             "with a caller-supplied d_work";
   }
   return "unknown error";
 }

@@ -15,10 +15,13 @@
 #include <cuda_runtime.h>
 
 #include <cstdint>
+#include <mutex>
 
 #include "../../include/apic.h"
 
 namespace apic {
+void note_cuda_error(cudaError_t e, const char* what);   // api.cu: fills the text apic_last_cuda_error() returns
+
 namespace {
 
 constexpr int kCorrChunks = 16;   // CTAs per (tile, direction): the overlap's lines are dealt round-robin to the chunks
@@ -192,6 +195,75 @@ int apic_reassemble(const float* d_fields, int tiles_y, int tiles_x, int tile_px
     blend_kernel<1><<<dim3((W + 255) / 256, gy), 256, 0, s>>>(f, reinterpret_cast<const float2*>(d_factors), tiles_y, tiles_x, T,
                                                              overlap, H, W, reinterpret_cast<float2*>(d_fov));
   return cudaGetLastError() == cudaSuccess ? APIC_OK : APIC_ECUDA;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// apic_reassemble_static: the same three kernels, for callers that have no way to hand over a d_work buffer.
+//
+// Who that is: code that runs where device memory can no longer be requested - a reassembly step that sits inside a
+// host application whose memory was handed out in full at start-up (an acquisition loop with a fixed arena, a plugin
+// whose host owns the allocator), or a latency-bound loop in which a cudaMalloc would stall every stream of the
+// process.  For them the correlation partial sums and the fp64 unit factors live in an array that is part of the
+// library image itself: it exists on a GPU from the moment the library's device code is loaded there and until the
+// process exits, whether or not it is ever used, so its size is a hard limit, kept modest.
+//
+// `g_reassemble_scratch` below is, on the host side of this file, only a handle that the CUDA runtime knows how to
+// look up.  It is NOT the device address (a kernel that were passed `g_reassemble_scratch` from host code would read
+// some host location, or fault); the device address is asked for once per device with cudaGetSymbolAddress while that
+// device is current, and that address is what the kernels get.
+// ---------------------------------------------------------------------------------------------------------------------
+#define APIC_REASSEMBLE_STATIC_MAX_TILES 1024   /* 1024 x (2 x 16 + 1) x 16 B = 528 KiB on every GPU that loads libapic */
+
+static __device__ __align__(256) double2 g_reassemble_scratch[size_t(APIC_REASSEMBLE_STATIC_MAX_TILES) *
+                                                              (2 * apic::kCorrChunks + 1)];
+
+namespace apic {
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mutex;
+double2* g_static_scratch_of_device[kStaticMaxDevices] = {};   // device address of g_reassemble_scratch, per device
+
+// Device address of the scratch on the CURRENT device (looked up at the first call on that device, then cached).
+int static_scratch(double2** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) { note_cuda_error(e, "apic_reassemble_static: cudaGetDevice"); return APIC_ECUDA; }
+  if (dev < 0 || dev >= kStaticMaxDevices) return APIC_EINVAL;
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  if (!g_static_scratch_of_device[dev]) {
+    double2* p = nullptr;
+    e = cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_reassemble_scratch);
+    if (e != cudaSuccess || !p) {
+      note_cuda_error(e, "apic_reassemble_static: cudaGetSymbolAddress(g_reassemble_scratch)");
+      return APIC_ECUDA;
+    }
+    g_static_scratch_of_device[dev] = p;
+  }
+  *out = g_static_scratch_of_device[dev];
+  return APIC_OK;
+}
+
+}  // namespace
+}  // namespace apic
+
+extern "C" {
+
+int apic_reassemble_static_max_tiles(void) { return APIC_REASSEMBLE_STATIC_MAX_TILES; }
+
+int apic_reassemble_static(const float* d_fields, int tiles_y, int tiles_x, int tile_px, int overlap, int align,
+                           float* d_fov, float* d_factors, void* cuda_stream) {
+  if (tiles_y < 1 || tiles_x < 1) return APIC_EINVAL;
+  if (size_t(tiles_y) * size_t(tiles_x) > size_t(APIC_REASSEMBLE_STATIC_MAX_TILES)) return APIC_ESCRATCH;
+  double2* work = nullptr;
+  const int rc = apic::static_scratch(&work);
+  if (rc != APIC_OK) return rc;
+  // Nothing in the scratch has to start at zero: overlap_corr_kernel stores every partial sum that phase_scan_kernel
+  // adds up (a zero where a tile has no left / upper neighbour), and the scan writes each factor before it reads it.
+  // What an earlier call left behind is therefore never looked at, and no clearing pass is enqueued.
+  return apic_reassemble(d_fields, tiles_y, tiles_x, tile_px, overlap, align, d_fov, d_factors, work, cuda_stream);
 }
 
 }  // extern "C"
