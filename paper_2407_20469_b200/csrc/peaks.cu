@@ -33,10 +33,17 @@ __global__ void __launch_bounds__(512) peak_smem_kernel(float* out, int iters) {
   __syncthreads();
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
   int idx = threadIdx.x;
+  const unsigned base = static_cast<unsigned>(__cvta_generic_to_shared(sh));
   for (int it = 0; it < iters; ++it) {
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
-      const float4 v = sh[(idx + k * 512) & 2047];                   // conflict-free LDS.128
+      // eight DISTINCT entries per iteration (offsets k * 256 of a 2048-entry ring; k * 512 made k and k + 4 the same
+      // address and let the compiler issue four loads for eight), each a volatile conflict-free LDS.128 that cannot be
+      // merged or hoisted: the count of loads executed is the count the rate is computed from
+      float4 v;
+      asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];"
+                   : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                   : "r"(base + unsigned((idx + k * 256) & 2047) * 16u));
       acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
     }
     idx = (idx + 32) & 2047;
