@@ -110,8 +110,9 @@ typedef struct {
                             6 = df_mgrid.cu, the round-1 kernel (redundant CG vectors, plain
                                 loads).  Measured on config 2: 0 is the
                                 fastest, 4-6 are kept as named, parity-tested alternatives     */
-  int df_team;           /* CTAs per tile, 1..8; 0 = chosen from the pass size (as many as the
-                            pass leaves resident CTA slots for)                                 */
+  int df_team;           /* CTAs per tile: 1, 2, 4 or 8 (anything else is APIC_EINVAL); 0 = chosen
+                            from the pass size (as many as the pass leaves resident CTA slots
+                            for; the automatic choice may also take 5, which cannot be asked for) */
   int df_order;          /* order of the darkfield extension (PAPER.md:135 states none).  0 = one
                             LED after the other by ascending |kappa|, ties by input order; a bin
                             belongs to the first LED that solves it (reading R15, the default).
@@ -180,8 +181,8 @@ int apic_reconstruct(apic_plan* plan, const float* d_intensity, int batch, float
 
 /* Same call with HOST buffers (pinned or pageable): copies the inputs to the device, runs
  * apic_reconstruct, copies the results back and synchronises before returning.  Batches of >= 32
- * tiles are cut into sub-batches of >= 16 tiles that alternate between two workspace sets (the
- * second is allocated on first use) and two compute streams, with uploads and downloads on two
+ * tiles are cut into min(8, batch / 16) equal sub-batches (each >= 16 tiles) that alternate between two
+ * workspace sets (the second is allocated on first use) and two compute streams, with uploads and downloads on two
  * copy streams, so that copies in both directions overlap the kernels.  h_pupil may be NULL. */
 int apic_reconstruct_host(apic_plan* plan, const float* h_intensity, int batch, float* h_field,
                           float* h_zernike, float* h_pupil, int32_t* h_status, void* cuda_stream);
@@ -215,7 +216,12 @@ int apic_reconstruct_host_u16(apic_plan* plan, const uint16_t* h_raw, const floa
  * must stay valid and untouched until the wait returns; a slot must be waited for before it is
  * submitted to again (a busy slot is waited for implicitly).  Results are the bits of
  * apic_reconstruct on the same inputs.  With bg_mode != 0 a submit blocks until the batch's
- * background pass has run (see apic_reconstruct).  Not thread-safe per plan. */
+ * background pass has run (see apic_reconstruct).  Not thread-safe per plan.
+ * Mixing with the device-pointer entries: apic_reconstruct, apic_reconstruct_u16, apic_reconstruct_prior,
+ * apic_profile_begin (and apic_debug_copy for slot 0) use the same workspace as the pipeline slots, so each of them
+ * first completes every batch that is still in flight, exactly as apic_wait_host would (the results are then in
+ * the host buffers and a later apic_wait_host on that slot returns at once).  They never run beside a submitted
+ * batch; a caller who wants overlap keeps to one family of entries per plan, or uses two plans. */
 int apic_submit_host(apic_plan* plan, int slot, const float* h_intensity, int batch, float* h_field,
                      float* h_zernike, float* h_pupil, int32_t* h_status);
 int apic_submit_host_u16(apic_plan* plan, int slot, const uint16_t* h_raw, const float* h_scale, int batch,

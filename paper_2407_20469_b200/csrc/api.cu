@@ -120,6 +120,7 @@ bool apic_plan::alloc_set(WsSet& z) {
   w.gram_parts = (std::max(d.n_rows, d.n_grad) + kGramRows - 1) / kGramRows;
   const size_t n_led = std::max<size_t>(1, h.dark.size());
   bool ok = true;
+  const size_t first_alloc = allocs.size(), bytes_before = workspace_bytes;
   ok = ok && dalloc(&w.G, c * h.nb * size_t(h.kk_n) * h.kk_n, false);
   w.KP = nullptr;
   if (h.kk_n != h.n) ok = ok && dalloc(&w.KP, c * h.nb * nn, false);
@@ -144,6 +145,18 @@ bool apic_plan::alloc_set(WsSet& z) {
   ok = ok && dalloc(&z.bs.live_count, 1, false);
   ok = ok && cuda_ok(cudaMallocHost(reinterpret_cast<void**>(&z.h_live_count), sizeof(int32_t)), "cudaMallocHost");
   if (ok) ok = cuda_ok(cudaMemset(w.cg_iters, 0, c * n_led * sizeof(int32_t)), "cudaMemset");
+  if (!ok) {
+    // give back what this attempt got, so that a retry (the lazily allocated second set) does not strand it
+    const std::string why = g_cuda_err;                  // keep the first failure's text ("out of memory")
+    for (size_t k = first_alloc; k < allocs.size(); ++k) cudaFree(allocs[k]);
+    allocs.resize(first_alloc);
+    workspace_bytes = bytes_before;
+    if (z.h_live_count) { cudaFreeHost(z.h_live_count); z.h_live_count = nullptr; }
+    z.ws = Workspace{};
+    z.bs = BatchState{};
+    cudaGetLastError();
+    g_cuda_err = why;
+  }
   z.ready = ok;
   return ok;
 }
@@ -152,12 +165,26 @@ bool apic_plan::alloc_set(WsSet& z) {
 // are per device; a plan lives on the device that was current at apic_plan_create).
 struct DeviceGuard {
   int prev = -1;
+  bool ok = true;          // false: the plan's device could not be made current; the entry returns APIC_ECUDA
   explicit DeviceGuard(int dev) {
     if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
-    if (prev != dev) cudaSetDevice(dev); else prev = -1;
+    if (prev != dev) ok = cuda_ok(cudaSetDevice(dev), "cudaSetDevice(plan's device)"); else prev = -1;
+    if (!ok) prev = -1;
   }
   ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
+
+// The device-pointer entries run on workspace set 0 and share the launch counter and the profiler with the host
+// pipeline: a batch that apic_submit_host left in flight is completed first (its results are then in its host
+// buffers, and the caller's later apic_wait_host returns at once).
+static int drain_host_slots(apic_plan* plan) {
+  for (int q = 0; q < 2; ++q)
+    if (plan->slot[q].busy) {
+      const int rc = apic_wait_host(plan, q);
+      if (rc != APIC_OK) return rc;
+    }
+  return APIC_OK;
+}
 
 static void fill_info(const HostTables& h, apic_plan_info_t* info) {
   std::memset(info, 0, sizeof *info);
@@ -362,7 +389,7 @@ int apic_plan_create(const apic_params* p, apic_plan** out) {
     q.mx = L.mx; q.my = L.my;
     for (int st = 0; st <= kMaxUStrips; ++st)
       q.u_strip_off[st] = L.u_row_off[size_t(std::min(16 * st, L.u_nrow))];
-    if ((L.u_nrow + 15) / 16 > kMaxUStrips) ok = false;
+    // (L.u_nrow + 15) / 16 <= kMaxUStrips: checked by build_geometry
     q.accumulate = L.accumulate ? 1 : 0;
     q.n_avg = int(L.avg_f.size());
     ok = ok && plan->upload(&q.avg_f, L.avg_f);
@@ -489,6 +516,8 @@ int apic_reconstruct(apic_plan* plan, const float* d_intensity, int batch, float
                      float* d_pupil, int32_t* d_status, void* cuda_stream) {
   if (!plan || !d_intensity) return APIC_EINVAL;
   DeviceGuard guard(plan->pd.device);
+  if (!guard.ok) return APIC_ECUDA;
+  if (const int rc = drain_host_slots(plan)) return rc;
   return reconstruct_impl(plan, 0, ImgSrc{d_intensity, nullptr, nullptr}, batch, d_field, d_zernike, d_pupil, d_status,
                           static_cast<cudaStream_t>(cuda_stream));
 }
@@ -497,6 +526,8 @@ int apic_reconstruct_prior(apic_plan* plan, const float* d_intensity, const floa
                            float* d_zernike, float* d_pupil, int32_t* d_status, void* cuda_stream) {
   if (!plan || !d_intensity || !d_zernike_init) return APIC_EINVAL;
   DeviceGuard guard(plan->pd.device);
+  if (!guard.ok) return APIC_ECUDA;
+  if (const int rc = drain_host_slots(plan)) return rc;
   return reconstruct_impl(plan, 0, ImgSrc{d_intensity, nullptr, nullptr}, batch, d_field, d_zernike, d_pupil, d_status,
                           static_cast<cudaStream_t>(cuda_stream), d_zernike_init);
 }
@@ -505,6 +536,8 @@ int apic_reconstruct_u16(apic_plan* plan, const uint16_t* d_raw, const float* d_
                          float* d_zernike, float* d_pupil, int32_t* d_status, void* cuda_stream) {
   if (!plan || !d_raw || !d_scale) return APIC_EINVAL;
   DeviceGuard guard(plan->pd.device);
+  if (!guard.ok) return APIC_ECUDA;
+  if (const int rc = drain_host_slots(plan)) return rc;
   return reconstruct_impl(plan, 0, ImgSrc{nullptr, d_raw, d_scale}, batch, d_field, d_zernike, d_pupil, d_status,
                           static_cast<cudaStream_t>(cuda_stream));
 }
@@ -533,6 +566,7 @@ static int reconstruct_host_impl(apic_plan* plan, const float* h_intensity, cons
   if (!plan || !h_field || !h_zernike || !h_status) return APIC_EINVAL;
   if (batch < 1 || batch > plan->params.max_batch) return APIC_EBATCH;
   DeviceGuard guard(plan->pd.device);
+  if (!guard.ok) return APIC_ECUDA;
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   const DevTables& t = plan->dev;
   const size_t nn = size_t(t.n) * t.n, on = size_t(t.n) * t.u;
@@ -652,6 +686,7 @@ static int submit_host_impl(apic_plan* plan, int slot, const float* h_intensity,
   if (!plan || !h_field || !h_zernike || !h_status || slot < 0 || slot > 1) return APIC_EINVAL;
   if (batch < 1 || batch > plan->params.max_batch) return APIC_EBATCH;
   DeviceGuard guard(plan->pd.device);
+  if (!guard.ok) return APIC_ECUDA;
   apic_plan::HostSlot& q = plan->slot[slot];
   if (q.busy) {                                          // a slot holds one batch at a time
     const int rc = apic_wait_host(plan, slot);
@@ -730,6 +765,7 @@ int apic_wait_host(apic_plan* plan, int slot) {
   apic_plan::HostSlot& q = plan->slot[slot];
   if (!q.busy) return APIC_OK;
   DeviceGuard guard(plan->pd.device);
+  if (!guard.ok) return APIC_ECUDA;
   q.busy = false;
   return cuda_ok(cudaEventSynchronize(q.out_done), "apic_wait_host") ? APIC_OK : APIC_ECUDA;
 }
@@ -754,6 +790,10 @@ int apic_debug_copy(const apic_plan* plan, int which, void* d_dst, int tiles, vo
   const int rc = apic_debug_buffer(plan, which, &src, &bytes);
   if (rc != APIC_OK) return rc;
   if (!d_dst || tiles < 1 || tiles > plan->chunk) return APIC_EINVAL;
+  DeviceGuard guard(plan->pd.device);
+  if (!guard.ok) return APIC_ECUDA;
+  // the stage buffers are those of workspace set 0: a batch in flight in pipeline slot 0 would be overwriting them
+  if (plan->slot[0].busy && apic_wait_host(const_cast<apic_plan*>(plan), 0) != APIC_OK) return APIC_ECUDA;
   if (!cuda_ok(cudaMemcpyAsync(d_dst, src, bytes * tiles, cudaMemcpyDeviceToDevice, static_cast<cudaStream_t>(cuda_stream)),
                "apic_debug_copy"))
     return APIC_ECUDA;
@@ -816,6 +856,9 @@ const char* apic_profile_category_name(int cat) { return (cat >= 0 && cat < CAT_
 
 int apic_profile_begin(apic_plan* plan, int stride, int max_samples) {
   if (!plan || stride < 1 || max_samples < 1) return APIC_EINVAL;
+  DeviceGuard guard(plan->pd.device);
+  if (!guard.ok) return APIC_ECUDA;
+  if (const int rc = drain_host_slots(plan)) return rc;   // the counters are per plan, not per batch in flight
   Profiler& pr = plan->prof;
   while (int(pr.ev.size()) < 2 * max_samples) {
     cudaEvent_t e;
@@ -834,6 +877,8 @@ int apic_profile_begin(apic_plan* plan, int stride, int max_samples) {
 
 int apic_profile_work(apic_plan* plan, unsigned long long* line_transforms) {
   if (!plan || !line_transforms) return APIC_EINVAL;
+  DeviceGuard guard(plan->pd.device);
+  if (!guard.ok) return APIC_ECUDA;
   *line_transforms = 0;
   for (WsSet& z : plan->set) {
     unsigned long long v = 0;
@@ -846,6 +891,8 @@ int apic_profile_work(apic_plan* plan, unsigned long long* line_transforms) {
 
 int apic_profile_end(apic_plan* plan, double* ms_sum, long long* samples, long long* launches) {
   if (!plan || !ms_sum || !samples || !launches) return APIC_EINVAL;
+  DeviceGuard guard(plan->pd.device);
+  if (!guard.ok) return APIC_ECUDA;
   Profiler& pr = plan->prof;
   pr.on = false;
   for (int c = 0; c < CAT_COUNT; ++c) { ms_sum[c] = 0; samples[c] = 0; launches[c] = pr.launches[c]; }

@@ -911,7 +911,12 @@ void launch_darkfield_tma(const DevTables& t, const DarkDev* d_leds, const DarkD
   cfg.gridDim = dim3(unsigned(G) * unsigned(teams));
 #ifdef APIC_TIMELINE
   // debugging aid (build with -DAPIC_TIMELINE): APIC_DF_TIMELINE=<file> dumps the clock64 marks of team 0
-  const char* tl_path = getenv("APIC_DF_TIMELINE");
+#if defined(APIC_DF_KNOBS) || defined(APIC_TIMELINE)
+  static const char* const tl_env = getenv("APIC_DF_TIMELINE");
+#else
+  static constexpr const char* tl_env = nullptr;        // the shipped library reads no environment variable
+#endif
+  const char* tl_path = tl_env;
   unsigned long long* dbg = nullptr;
   if (tl_path) {
     cudaMalloc(&dbg, size_t(kMaxTeam) * kTlCap * sizeof(unsigned long long));

@@ -1,4 +1,5 @@
-// df_wide.cu - S8-S10 darkfield extension on per-LED reduced cyclic grids, "wide" scheduling (df_mode 5 at N = 256).
+// df_wide.cu - S8-S10 darkfield extension on per-LED reduced cyclic grids, "wide" scheduling: the default darkfield kernel at N = 256
+// (df_mode 0: 256-thread CTAs at 128 registers; df_mode 5: its 1024-thread shape, a measured alternative).
 //
 // Same mathematics as df_mgrid.cu (Eq. 11-13; readings R15-R17, B1): per darkfield LED, conjugate
 // gradients on the normal equations of  C u = d,  C[k,u] = conj P_hat(u - k), k in Q, u in U, with C and C^H applied by
@@ -29,6 +30,7 @@
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
+#include <mutex>
 #include <vector>
 
 #include "fft_xy.cuh"
@@ -69,7 +71,7 @@ struct Args {
   const int32_t* live_count;
   int chunk0, n_tiles;
   unsigned long long* work;   // executed nominal flop (5 L log2 L per line transform)
-  unsigned long long* tl;     // optional timeline of team 0 (APIC_DF_TIMELINE=<file>): [cta][group][kTlCap] clock marks
+  unsigned long long* tl;     // optional timeline of team 0 (-DAPIC_DF_KNOBS builds: APIC_DF_TIMELINE=<file>): [cta][group][kTlCap] clock marks
 };
 constexpr int kTlCap = 8192;
 #ifdef APIC_TIMELINE   // debugging aid: build with APIC_EXTRA_NVCC_FLAGS=-DAPIC_TIMELINE, run with APIC_DF_TIMELINE=<file>
@@ -1210,6 +1212,42 @@ __global__ void __launch_bounds__(NG * GT, MINB) df_wide_kernel(const __grid_con
   if (g.tid == 0 && flop > 0.0) atomicAdd(a.work, (unsigned long long)(flop + 0.5));
 }
 
+// Developer knobs (APIC_DF_NO_VR, APIC_DF_WIDE_DEBUG, APIC_DF_TIMELINE, APIC_DF_WIDE_NG) exist only in a build with
+// APIC_EXTRA_NVCC_FLAGS=-DAPIC_DF_KNOBS (or -DAPIC_TIMELINE); the shipped library reads no environment variable.  Read
+// once per process.
+#if defined(APIC_DF_KNOBS) || defined(APIC_TIMELINE)
+static const char* knob(int which) {
+  static const char* const v[4] = {getenv("APIC_DF_NO_VR"), getenv("APIC_DF_WIDE_DEBUG"), getenv("APIC_DF_TIMELINE"),
+                                   getenv("APIC_DF_WIDE_NG")};
+  return v[which];
+}
+#else
+static constexpr const char* knob(int) { return nullptr; }
+#endif
+enum { KNOB_NO_VR = 0, KNOB_DEBUG = 1, KNOB_TIMELINE = 2, KNOB_NG = 3 };
+
+// cudaFuncSetAttribute is per device and per kernel instantiation: done when the shared-memory size first grows past
+// what was set (device, instantiation) - not on every pass of the hot path.
+template <int NG, int MINB>
+static bool ensure_attributes(int device, size_t smem) {
+  constexpr int kMaxDev = 64;
+  static size_t set_smem[kMaxDev] = {};
+  static std::mutex mu;
+  if (device < 0 || device >= kMaxDev) return false;
+  std::lock_guard<std::mutex> lock(mu);
+  if (set_smem[device] >= smem && set_smem[device] != 0) return true;
+  auto kern = df_wide_kernel<NG, MINB>;
+  const cudaError_t e1 = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
+  const cudaError_t e2 = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+  if (e1 != cudaSuccess || e2 != cudaSuccess) {
+    if (knob(KNOB_DEBUG)) fprintf(stderr, "df_wide: attr %s / %s\n", cudaGetErrorString(e1), cudaGetErrorString(e2));
+    cudaGetLastError();
+    return false;
+  }
+  set_smem[device] = smem;
+  return true;
+}
+
 template <int NG, int MINB>
 static bool launch_ng(const Args& a0, const DarkDev* h_leds, int n_leds, const LaunchCtx& c, int G, int sms) {
   Args a = a0;
@@ -1233,7 +1271,7 @@ static bool launch_ng(const Args& a0, const DarkDev* h_leds, int n_leds, const L
   while (nvec > 1 && smem_for(nvec) > size_t(227 * 1024)) --nvec;
   size_t smem = smem_for(nvec);
   a.vr = 0;
-  if (NG == 4 && G == 2 && !getenv("APIC_DF_NO_VR")) {
+  if (NG == 4 && G == 2 && !knob(KNOB_NO_VR)) {
     // decimated CG loop: w of the set-up in global memory, the CG region holds four redundant vectors of max_unknown
     int mu = 2;
     for (int k = 0; k < n_leds; ++k) mu = std::max(mu, h_leds[k].n_unknown);
@@ -1243,14 +1281,12 @@ static bool launch_ng(const Args& a0, const DarkDev* h_leds, int n_leds, const L
     if (sm <= size_t(227 * 1024)) { a.vr = 1; a.vr_mu = mu; nvec = 1; smem = sm; }
   }
   a.vec_global = nvec == 4 ? 0 : nvec == 3 ? 4 : nvec == 2 ? 6 : 7;
-  const bool dbg = getenv("APIC_DF_WIDE_DEBUG") != nullptr;
+  const bool dbg = knob(KNOB_DEBUG) != nullptr;
   if (dbg) fprintf(stderr, "df_wide: NG %d G %d kex %d kpc %d cap %d smem %zu\n", NG, G, a.kex, a.kpc, a.cap, smem);
   if (dbg) fprintf(stderr, "df_wide: vec_global %d\n", a.vec_global);
   if (smem > size_t(227 * 1024)) return false;
   auto kern = df_wide_kernel<NG, MINB>;
-  cudaError_t e1 = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem));
-  cudaError_t e2 = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-  if (dbg && (e1 != cudaSuccess || e2 != cudaSuccess)) fprintf(stderr, "df_wide: attr %s / %s\n", cudaGetErrorString(e1), cudaGetErrorString(e2));
+  if (!ensure_attributes<NG, MINB>(c.pd->device, smem)) return false;   // nothing pending: the caller may fall back
   cudaLaunchConfig_t cfg{};
   cudaLaunchAttribute at[2];
   at[0].id = cudaLaunchAttributeClusterDimension;
@@ -1274,7 +1310,7 @@ static bool launch_ng(const Args& a0, const DarkDev* h_leds, int n_leds, const L
   }
   const int teams = std::max(1, std::min(max_clusters, c.chunk_tiles));
   cfg.gridDim = dim3(unsigned(G) * unsigned(teams));
-  const char* tl_path = getenv("APIC_DF_TIMELINE");
+  const char* tl_path = knob(KNOB_TIMELINE);
   const size_t tl_words = size_t(G) * NG * kTlCap;
   if (tl_path) {
     cudaMalloc(&a.tl, tl_words * sizeof(unsigned long long));
@@ -1285,6 +1321,8 @@ static bool launch_ng(const Args& a0, const DarkDev* h_leds, int n_leds, const L
     ProfScope ps(c, CAT_DF_WIDE);
     ok = cudaLaunchKernelEx(&cfg, kern, a) == cudaSuccess;
   }
+  // A failed launch enqueued nothing; clear its error so that the caller's fallback kernel is judged on its own.
+  if (!ok) cudaGetLastError();
   if (tl_path) {                                         // debugging aid: marks of team 0, one line per mark: cta group ns id
     std::vector<unsigned long long> h(tl_words);
     cudaStreamSynchronize(c.stream);
@@ -1325,7 +1363,7 @@ bool launch_darkfield_wide(const DevTables& t, const DarkDev* d_leds, const Dark
   const int sms = c.pd->sms;
   int ng = groups > 0 ? groups : 4;   // 4, 2, 1: groups per CTA at 64 registers; 11: one group at 128 registers
   if (groups != 11)
-    if (const char* e = getenv("APIC_DF_WIDE_NG")) ng = atoi(e);   // experiments with the shapes of mode 5
+    if (const char* e = knob(KNOB_NG)) ng = atoi(e);   // experiments with the shapes of mode 5 (-DAPIC_DF_KNOBS builds)
   int G = team_size;
   if (G <= 0) {
     // NG = 4: pairs of 1024-thread CTAs, one CTA per SM (the decimated CG loop needs exactly this shape; larger passes

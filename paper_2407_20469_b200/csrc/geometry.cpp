@@ -358,6 +358,11 @@ bool build_geometry(const apic_params& p, HostTables& t, std::string& err) {
     };
     bbox(d, L.d_col0, L.d_ncol, L.d_row0, L.d_nrow);
     bbox(U, L.u_col0, L.u_ncol, L.u_row0, L.u_nrow);
+    if ((L.u_nrow + 15) / 16 > kMaxUStrips) {
+      snprintf(buf, sizeof buf, "darkfield LED %d: its unknown set spans %d rows, more than the %d the darkfield kernels' strip "
+               "table holds (pupil radius too large for this tile_n)", led, L.u_nrow, 16 * kMaxUStrips);
+      err = buf; return false;
+    }
     bbox(Q, L.q_col0, L.q_ncol, L.q_row0, L.q_nrow);
     // disc entries: U first (row-major), then P (row-major)
     std::vector<int32_t> ent(size_t(n) * n, -1);

@@ -14,6 +14,10 @@
 
 namespace apic {
 
+// The darkfield kernels walk the rows of an LED's unknown set U in strips of 16; their per-LED strip table has this many
+// entries.  A disc spans <= 2R + 1 <= 0.34 N rows: <= 11 strips at N = 512.  build_geometry rejects what does not fit.
+constexpr int kMaxUStrips = 16;
+
 struct DarkLed {
   int led = 0;                 // input index
   double kappa[2] = {0, 0};

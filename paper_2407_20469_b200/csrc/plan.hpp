@@ -43,7 +43,6 @@ struct DevTables {
   const float* pupil_zern;       // [n_pupil][nz]
 };
 
-constexpr int kMaxUStrips = 16;            // a disc spans <= 2R + 1 <= 0.34 N rows: <= 11 strips of 16 rows at N = 512
 
 struct DarkDev {
   int n_unknown, n_disc, n_eq;
