@@ -49,6 +49,8 @@ def parse_args():
     ap.add_argument("--impl", default="apic", choices=["apic", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index (2 = default workload)")
     ap.add_argument("--tiles", type=int, default=0, help="tiles per step and per GPU (0 = the config's batch, capped at 64)")
+    ap.add_argument("--distinct-tiles", type=int, default=0, help="distinct seeded tiles generated per GPU and repeated to fill "
+                    "the step (0 = every tile of the step distinct)")
     ap.add_argument("--chunk", type=int, default=0, help="apic_params.chunk_tiles (0 = library default)")
     ap.add_argument("--df-mode", type=int, default=0, help="darkfield kernel (apic.h): 0 default (df_wide.cu, 256-thread CTAs at 128 registers), "
                     "3 full grid, 4 async-proxy staging, 5 1024-thread CTA pairs with the decimated CG loop, 6 the round-1 kernel")
@@ -61,13 +63,11 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--breakdown", action="store_true", help="also print the per-kernel time table to stderr")
     ap.add_argument("--ncu-summary", default="", help="no run: append the kernels of an `ncu -i <rep> --page raw --csv` dump "
-                    "to profiles/r2_ncu_kernels.csv (with --commit and --workload)")
+                    "to profiles/r3_ncu_kernels.csv (with --commit and --workload)")
     ap.add_argument("--commit", default="", help="--ncu-summary: the commit the capture was taken at")
     ap.add_argument("--workload", default="", help="--ncu-summary: workload tag, e.g. cfg2_64tiles")
     ap.add_argument("--reassemble", action="store_true", help="no reconstruction: time apic_reassemble (within-FOV reassembly of "
                     "5 x 5 tiles of 768 x 768 output pixels with 10 %% overlap) against the HBM roofline")
-    ap.add_argument("--dense-probe", action="store_true", help="no run of the library: time the dense route of the darkfield "
-                    "step (G = C^H C with the library GEMM on tensor cores) for the shapes of config 2")
     return ap.parse_args()
 
 
@@ -212,10 +212,10 @@ def kernel_short_name(full):
 
 def ncu_capture(kernel, workload):
     """Per-launch DRAM bytes and shared-memory wavefronts of `kernel` from the committed ncu --set full summary
-    (profiles/r2_ncu_kernels.csv).  A row taken with other kernel sources than the ones in the tree is refused."""
+    (profiles/r3_ncu_kernels.csv).  A row taken with other kernel sources than the ones in the tree is refused."""
     import csv
     try:
-        with open(os.path.join(ROOT, "profiles", "r2_ncu_kernels.csv")) as fh:
+        with open(os.path.join(ROOT, "profiles", "r3_ncu_kernels.csv")) as fh:
             rows = [r for r in csv.DictReader(fh) if r["kernel"] == kernel and r["workload"] == workload]
     except Exception:
         return None
@@ -230,7 +230,7 @@ def ncu_capture(kernel, workload):
 
 def ncu_summary(args):
     """Reduces an `ncu --page raw --csv` dump of an `ncu --set full` capture to one row per kernel launch in
-    profiles/r2_ncu_kernels.csv: what bench.py's roofline line reads (traffic, smem_frac) plus the figures DESIGN.md
+    profiles/r3_ncu_kernels.csv: what bench.py's roofline line reads (traffic, smem_frac) plus the figures DESIGN.md
     quotes (issue-slot utilisation, occupancy, L2 hit rate, stall shares)."""
     import csv
     with open(args.ncu_summary) as fh:
@@ -248,7 +248,7 @@ def ncu_summary(args):
             x *= {"Mbyte": 1e6, "Gbyte": 1e9, "Kbyte": 1e3, "byte": 1.0, "us": 1e-3, "ns": 1e-6, "ms": 1.0, "s": 1e3}.get(u, 1.0)
         return x
 
-    out_path = os.path.join(ROOT, "profiles", "r2_ncu_kernels.csv")
+    out_path = os.path.join(ROOT, "profiles", "r3_ncu_kernels.csv")
     fields = ["kernel", "workload", "commit", "source_hash", "duration_ms", "dram_bytes_read", "dram_bytes_write",
               "smem_wavefronts", "inst_executed", "issue_active_pct", "warps_active_pct", "l2_hit_pct", "registers",
               "dyn_smem_bytes", "grid", "cluster", "stall_barrier_pct", "stall_long_sb_pct", "stall_short_sb_pct",
@@ -283,55 +283,6 @@ def ncu_summary(args):
                         "stall_wait_pct": f"{100 * stall.get('wait', 0) / tot:.1f}",
                         "stall_membar_pct": f"{100 * stall.get('membar', 0) / tot:.1f}"})
             print("appended", name, args.workload, "to", out_path)
-
-
-def dense_probe():
-    """The dense route of the darkfield step, for DESIGN.md section 7 (north_star: tensor cores only if the contraction
-    dominates): PAPER.md:135 builds the block-Toeplitz C explicitly (|Q| x |U| complex per LED); its normal matrix
-    G = C^H C is a contraction over |Q|.  Times G for ONE darkfield LED of each of 64 tiles with the library GEMM
-    (cuBLAS through torch.bmm; complex = 4 real products) in fp32 and on the tensor cores in TF32 (one pass: 10-bit
-    mantissas, too coarse for the 1e-3 band tolerance; fp32-level accuracy needs 3 passes), plus the Cholesky factor."""
-    import torch
-    torch.cuda.set_device(0)
-
-    def timeit(f, n=5):
-        for _ in range(2):
-            f()
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        for _ in range(n):
-            f()
-        e1.record()
-        torch.cuda.synchronize()
-        return e0.elapsed_time(e1) / n
-
-    tiles, res = 64, {}
-    for name, (nq, nu) in {"ring_0.30": (8624, 569), "ring_0.40": (7908, 1194)}.items():   # |Q| x |U| of config 2's plan
-        cr = torch.randn(tiles, nq, nu, device="cuda")
-        ci = torch.randn(tiles, nq, nu, device="cuda")
-        flop = 4 * 2.0 * tiles * nq * nu * nu
-        row = {"Q": nq, "U": nu, "tiles": tiles}
-        for mode, tf32 in (("fp32", False), ("tf32_1pass", True)):
-            torch.backends.cuda.matmul.allow_tf32 = tf32
-
-            def gram():
-                a = torch.bmm(cr.transpose(1, 2), cr)
-                a += torch.bmm(ci.transpose(1, 2), ci)
-                b = torch.bmm(cr.transpose(1, 2), ci)
-                b -= torch.bmm(ci.transpose(1, 2), cr)
-                return a, b
-            ms = timeit(gram)
-            row[mode] = {"ms_per_led": ms, "tflops_real": flop / ms / 1e9}
-        torch.backends.cuda.matmul.allow_tf32 = False
-        g = torch.randn(tiles, nu, nu, dtype=torch.complex64, device="cuda")
-        g = g @ g.conj().transpose(1, 2) + nu * torch.eye(nu, device="cuda", dtype=torch.complex64)
-        row["cholesky_ms_per_led"] = timeit(lambda: torch.linalg.cholesky(g), n=2)
-        res[name] = row
-        del cr, ci, g
-    step = sum(8 * (r["tf32_1pass"]["ms_per_led"] + r["cholesky_ms_per_led"]) for r in res.values())
-    print(json.dumps({"dense_probe": res, "ms_per_64_tile_step_tf32_1pass": step,
-                      "note": "8 LEDs per ring; building C and the right-hand sides not included"}), flush=True)
 
 
 def reassemble_bench(args):
@@ -394,9 +345,6 @@ def main():
         return
     if args.reassemble:
         reassemble_bench(args)
-        return
-    if args.dense_probe:
-        dense_probe()
         return
     from apic_synth import get_config, make_batch, plan_args
     cfg = get_config(args.config)
@@ -472,12 +420,12 @@ def roofline_line(ctx, plan, prof, clocks, tiles, workload, step_ms, algo_hbm_by
         cap = ncu_capture(dominant, workload)
         traffic, smem_frac, cap_note = None, None, "no ncu --set full capture of this kernel and workload under profiles/"
         if cap and cap.get("stale"):
-            cap_note = "profiles/r2_ncu_kernels.csv was captured with other kernel sources (hash mismatch): refused"
+            cap_note = "profiles/r3_ncu_kernels.csv was captured with other kernel sources (hash mismatch): refused"
         elif cap:
             traffic = cap["dram_bytes"]
             # 128 bytes per shared-memory wavefront, against the measured shared-memory read bandwidth
             smem_frac = cap["smem_wavefronts"] * 128.0 / (cap["duration_ms"] * 1e-3) / (mp["smem_tbs"] * 1e12)
-            cap_note = f"ncu --set full at commit {cap['commit']} (profiles/r2_ncu_kernels.csv), per launch"
+            cap_note = f"ncu --set full at commit {cap['commit']} (profiles/r3_ncu_kernels.csv), per launch"
         out.update({"bound": "alu", "achieved": achieved, "peak": mp["fp32_fma_tflops"], "unit": "TFLOP/s",
                     "frac": (achieved / mp["fp32_fma_tflops"]) if achieved else None,
                     "frac_of_fadd_peak": (achieved / mp["fp32_fadd_tflops"]) if achieved else None,
@@ -505,11 +453,19 @@ def run_batch(ctx):
     args, cfg, torch, A, rank, world, local, dist = (ctx[k] for k in ("args", "cfg", "torch", "A", "rank", "world", "local", "dist"))
     from apic_synth import make_batch, plan_args
     tiles = args.tiles or min(cfg.batch, 64)
-    # seeded synthetic tiles of this rank (weak scaling: every GPU gets its own `tiles` tiles); a few
-    # distinct tiles are generated and repeated to fill the batch, each GPU starting at another tile
-    n_gen = min(tiles, 8)
+    # seeded synthetic tiles of this rank (weak scaling: every GPU gets its own `tiles` tiles), every tile of the step
+    # distinct (generated on the host, outside every timed region; --distinct-tiles M repeats M tiles to fill the
+    # batch, for quick runs), each GPU starting at another tile
+    n_gen = min(tiles, args.distinct_tiles or tiles, max(1, cfg.batch))
     base = (rank * n_gen) % max(1, cfg.batch - n_gen + 1)
-    stacks, truths = make_batch(cfg, range(base, base + n_gen))
+    if n_gen > 8:
+        # tiles are seeded per index, so generating them side by side on the host threads changes nothing but the wait
+        import concurrent.futures as cf
+        with cf.ThreadPoolExecutor(max_workers=min(16, host_threads())) as ex:
+            made = list(ex.map(lambda t: make_batch(cfg, [t]), range(base, base + n_gen)))
+        stacks, truths = np.concatenate([m[0] for m in made]), [m[1][0] for m in made]
+    else:
+        stacks, truths = make_batch(cfg, range(base, base + n_gen))
     reps = -(-tiles // n_gen)
     host = np.concatenate([stacks] * reps)[:tiles]
     x = torch.from_numpy(host).cuda()
@@ -597,7 +553,7 @@ def run_batch(ctx):
         assert all(np.array_equal(o[0].numpy(), ref_field) for o in outs), "streaming host entry and device entry disagree"
         d2h = int(hf.numel() * 8 + hz.numel() * 4 + hp.numel() * 8 + hs.numel() * 4)
         e2e = {"value": world * k2 * tiles * on * on / 1e6 / dt, "unit": UNIT, "h2d_bytes_per_step": int(hx.numel() * 4),
-               "d2h_bytes_per_step": d2h, "steps": k2,
+               "d2h_bytes_per_step": d2h, "steps": k2, "input": "fp32 intensities",
                "api": "apic_submit_host / apic_wait_host (pinned host buffers, fp32 intensities, two batches in flight)"}
         # (2) one blocking call per step: upload, kernels and download of a step overlap only inside the call
         dt = timed(lambda i: plan.reconstruct_host(hx, hf, hz, hp, hs, stream))
@@ -619,6 +575,13 @@ def run_batch(ctx):
             dt = timed(lambda i: plan.reconstruct_host_u16(hr, hsc, hf, hz, hp, hs, stream))
             e2e["u16"]["single_call"] = {"value": world * k2 * tiles * on * on / 1e6 / dt, "unit": UNIT,
                                          "api": "apic_reconstruct_host_u16 (blocking)"}
+            # BASELINE.json states this workload as "uint16 raw converted to fp32": what a user uploads is the camera's
+            # counts, so the uint16 streaming entry is the declared end-to-end number and the fp32-host one sits beside it
+            f32 = {k: e2e[k] for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "api", "single_call")}
+            u16 = e2e["u16"]
+            e2e = {"value": u16["value"], "unit": UNIT, "h2d_bytes_per_step": u16["h2d_bytes_per_step"],
+                   "d2h_bytes_per_step": d2h, "steps": k2, "input": "uint16 counts + per-image fp32 scale",
+                   "api": u16["api"], "single_call": u16["single_call"], "f32": f32}
 
     # ---- the oracle on this box's host cores (rank 0, N = 1 only): one tile of the same workload
     cpu = None

@@ -79,7 +79,11 @@ typedef struct {
                             the transform work of S1-S5                                          */
   int refine_iters;      /* re-wrapped refinements of the aberration fit (R11); 0..16   */
   int df_iters;          /* maximum CGLS iterations per darkfield LED (>= 1)                      */
-  float df_tol;          /* CGLS stops when ||C^H r|| <= df_tol * ||C^H d||; 0 = run df_iters     */
+  float df_tol;          /* CGLS stops when ||C^H r|| <= df_tol * ||C^H d||; 0 = run df_iters.
+                            (There is no df_solver field: SURVEY.md 8(b) listed one for a dense
+                            Cholesky alternative; that route was measured at ~60x the cost of the
+                            matrix-free CG - DESIGN.md section 5, "The dense route" - and is not
+                            built, so a selector would have one legal value.)                    */
   float intensity_floor; /* I <- max(I, floor * mean(I)) before the log (R6)            */
   int bg_mode;           /* 0 off | 1: mean(I_bright) >= bg_threshold | 2: var/mean^2 <= thr      */
   float bg_threshold;
