@@ -6,7 +6,11 @@ Calls ONLY `oracle/` and the seeded generator `apic_synth/` (never the CUDA libr
 `lstsq` of Eq. 13 at N = 512 (up to 37,000 x 4,786 complex128 per LED) takes minutes per tile on a few
 cores, which is why the result is stored instead of recomputed by the GPU parity test.
 
-    python tests/golden/make_cfg3_golden.py            # about 7 min on 4 cores, <= 20 GB of memory
+    python tests/golden/make_cfg3_golden.py            # tile 0: about 7 min on 4 cores, <= 20 GB of memory
+    python tests/golden/make_cfg3_golden.py 1 2 3 4 5 6 7    # more tiles (>= 8 tiles of config 3)
+
+cfg3_tile0.npz holds everything; cfg3_tile<t>.npz for t > 0 hold only what differs from tile to tile (spectrum on the
+known region, coefficients, status, field sample): the index arrays are geometry and are read from tile 0's file.
 
 Stored (complex64 / float64): the object spectrum on the final known region (row-major order of the
 centred mask), the Zernike coefficients, the status, |U| and |Q| per darkfield LED in processing order,
@@ -28,16 +32,29 @@ from oracle import apic_oracle as O               # noqa: E402
 from helpers import oracle_params                 # noqa: E402
 
 
-def main():
+def main(tiles):
     cfg = get_config(3)
     t0 = time.time()
-    stack, _ = make_tile(cfg, 0)
     p = oracle_params(cfg)
     geo = O.Geometry(p)
     sets, known_final = O.darkfield_sets(geo)
     print(f"geometry {time.time() - t0:.0f} s: {len(sets)} darkfield LEDs, |known| = {int(known_final.sum())}", flush=True)
-    r = O.reconstruct_tile(stack, p, geo=geo, sets=sets, keep=True)
-    print(f"oracle {time.time() - t0:.0f} s, status {r.status}", flush=True)
+    for tile in tiles:
+        stack, _ = make_tile(cfg, tile)
+        r = O.reconstruct_tile(stack, p, geo=geo, sets=sets, keep=True)
+        print(f"tile {tile}: oracle {time.time() - t0:.0f} s, status {r.status}", flush=True)
+        if tile == 0:
+            write_full(geo, sets, r)
+        else:
+            assert np.array_equal(r.known, known_final)
+            np.savez_compressed(os.path.join(HERE, f"cfg3_tile{tile}.npz"),
+                                o_hat_known=r.o_hat[r.known].astype(np.complex64),
+                                zernike=np.asarray(r.zernike, dtype=np.float64), status=np.int32(r.status),
+                                field_sample=r.field[::64, ::64].astype(np.complex64))
+        print(f"tile {tile} written", flush=True)
+
+
+def write_full(geo, sets, r):
     ky, kx = np.nonzero(r.known)
     owner = np.full(r.known.shape, -1, dtype=np.int8)       # -1: union of the NA-matching discs; k: solved by the k-th darkfield LED
     for k, ds in enumerate(sets):
@@ -55,8 +72,7 @@ def main():
         n_equations=np.array([int(s.Q.sum()) for s in sets], dtype=np.int32),
         field_sample=r.field[::64, ::64].astype(np.complex64),
     )
-    print("written", flush=True)
 
 
 if __name__ == "__main__":
-    main()
+    main([int(a) for a in sys.argv[1:]] or [0])
